@@ -1,0 +1,186 @@
+/* slp_moe.h — C ABI of libslpmoe: one routed-MoE layer of stream-loading prefill (SLP) on one B200.
+ *
+ * The problem, as the paper states it: a layer's FP8 expert weights live in pinned host DRAM (the
+ * authoritative copy never leaves the host, §3.1 "the authoritative copy always
+ * remains in host memory"); a prompt chunk's hidden states are on the GPU; the module is executed
+ * on a stream in order with other modules while a loader stages its weights into GPU memory and
+ * signals readiness with events (§3.1, Fig. 5).  The module itself is
+ * gate -> sort -> expert FFNs -> weighted sum (Fig. 2 steps 3-5; PAPER.md:48 shared
+ * experts; Fig. 11 gate/up/down), on FP8 weights with block scales, activations
+ * quantised to FP8, FP32 accumulation (§2.2.5, PAPER.md:235,255 128-wide K blocks).
+ *
+ * Every step runs in hand-written CUDA kernels for sm_100a.  There is no CPU path: every entry
+ * point that needs the GPU returns SLP_ERR_CUDA when none is usable.
+ *
+ * Conventions
+ *  - All functions return slp_status (0 = ok, negative = error); slp_last_error() returns a
+ *    thread-local, NUL-terminated description of the last error on the calling thread.
+ *    No C++ exception crosses this boundary.
+ *  - "host" pointers are CPU addresses, "dev" pointers are CUDA device addresses on cfg.device.
+ *  - Tensors are dense row-major.  bf16 = 16-bit brain float bit patterns.  e4m3 = OCP FP8 E4M3
+ *    (bias 7, max 448, 0x7F/0xFF = NaN, no infinities).
+ *  - Shapes: hidden H and moe_intermediate I are multiples of 128; n_experts E divisible by
+ *    n_group; 1 <= top_k <= 32, top_k <= topk_group * E / n_group; E <= 512; n_shared in {0, 1}
+ *    with shared_intermediate == moe_intermediate.  Anything else: SLP_ERR_UNSUPPORTED_SHAPE at
+ *    create (never a silent fallback).
+ */
+#ifndef SLP_MOE_H
+#define SLP_MOE_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct slp_moe_layer slp_moe_layer; /* opaque handle */
+
+typedef enum {
+  SLP_OK = 0,
+  SLP_ERR_INVALID_ARG = -1,
+  SLP_ERR_UNSUPPORTED_SHAPE = -2,
+  SLP_ERR_CUDA = -3,
+  SLP_ERR_OOM = -4,
+  SLP_ERR_NOT_PINNED = -5,
+  SLP_ERR_BUSY = -6,
+  SLP_ERR_KERNEL_TIMEOUT = -7 /* an in-kernel pipeline wait exceeded its watchdog bound */
+} slp_status;
+
+typedef enum { SLP_STREAMED = 0, SLP_RESIDENT = 1 } slp_residency;
+typedef enum { SLP_SCORE_SIGMOID_BIAS = 0, SLP_SCORE_SOFTMAX = 1 } slp_scoring;
+
+/* Layer configuration (PAPER.md:48 gate; BASELINE.json configs for the constants). */
+typedef struct {
+  uint32_t struct_size;       /* = sizeof(slp_moe_cfg); ABI versioning */
+  int32_t device;             /* CUDA ordinal */
+  int32_t hidden;             /* H */
+  int32_t n_experts;          /* E routed experts */
+  int32_t top_k;              /* k */
+  int32_t n_group;            /* G contiguous expert groups (1 = no grouping) */
+  int32_t topk_group;         /* groups kept per token */
+  int32_t moe_intermediate;   /* I */
+  int32_t n_shared;           /* 0 or 1 shared expert, always active, weight 1 */
+  int32_t shared_intermediate;/* must equal moe_intermediate when n_shared == 1 */
+  int32_t scoring;            /* slp_scoring */
+  int32_t norm_topk;          /* 1: w_j = s_j / sum_j s_j * routed_scale; 0: w_j = s_j * routed_scale */
+  float routed_scale;
+  int32_t max_tokens;         /* workspace is sized for this T */
+  int32_t staging_slots;      /* streamed mode: expert slots in HBM, the paper's ring length
+                                 ("the number of experts of a layer" for short
+                                 prompts, 2 = ping-pong for very long ones).  0 = auto (= E).
+                                 Valid: 2..E. */
+  int32_t experts_per_launch; /* streamed mode: experts whose tiles one GEMM launch covers once
+                                 their copies have landed.  0 = auto.  Valid: 1..staging_slots/2
+                                 (or staging_slots when staging_slots == E). */
+  int32_t skip_empty_experts; /* 1: experts that received no token are neither copied nor run
+                                 (needs the counts on the host: one small D2H + sync inside
+                                 prefill).  0: paper-faithful fixed order, every expert copied. */
+  int32_t require_pinned;     /* 1: create fails with SLP_ERR_NOT_PINNED if a weight buffer is
+                                 pageable.  0: create pins it with cudaHostRegister. */
+  int32_t gemm_impl;          /* 0: tcgen05/TMEM/TMA grouped GEMM (the product path).
+                                 1: plain CUDA-core grouped GEMM kept for bring-up and for
+                                 triaging the tensor-core kernel; same kernels around it. */
+} slp_moe_cfg;
+
+/* Host weight pointers.  Borrowed for the lifetime of the handle; the host copy stays
+ * authoritative.  Routed expert weights stay on the host in streamed mode and are
+ * copied per call; router weights, bias, all fp32 block scales and the shared expert are uploaded
+ * once by create and stay resident (BASELINE.json config 1: shared expert "kept resident"). */
+typedef struct {
+  const float* router_w;            /* [E, H] fp32 */
+  const float* router_bias;         /* [E] fp32, or NULL (softmax scoring ignores it) */
+  const uint8_t* const* gate_q;     /* E pointers, each [I, H] e4m3 (K = H contiguous) */
+  const float* const* gate_s;       /* E pointers, each [I/128, H/128] fp32; w = decode(q) * s */
+  const uint8_t* const* up_q;       /* as gate */
+  const float* const* up_s;
+  const uint8_t* const* down_q;     /* E pointers, each [H, I] e4m3 (K = I contiguous) */
+  const float* const* down_s;       /* E pointers, each [H/128, I/128] fp32 */
+  const uint8_t* shared_gate_q;     /* [I, H] or NULL when n_shared == 0 */
+  const float* shared_gate_s;
+  const uint8_t* shared_up_q;
+  const float* shared_up_s;
+  const uint8_t* shared_down_q;     /* [H, I] */
+  const float* shared_down_s;
+} slp_moe_host_weights;
+
+/* Per-call statistics of the most recent completed slp_moe_prefill (CUDA-event times, ms). */
+typedef struct {
+  uint32_t struct_size;
+  int32_t tokens;
+  int32_t residency;
+  int32_t experts_copied;
+  int32_t experts_skipped;
+  int64_t bytes_copied;       /* host -> HBM bytes moved by the streaming engine */
+  float ms_total;             /* entry to exit on the caller's stream */
+  float ms_copy_span;         /* first H2D start to last H2D end on the copy stream (0 if resident) */
+  float ms_route;             /* router + histogram/scan/permute + hidden quantisation */
+  float ms_experts;           /* first expert GEMM launch to last (includes waits on copies) */
+  float ms_combine;
+  int32_t gemm_launches;      /* grouped-GEMM kernel launches in the call */
+  int32_t kernel_launches;    /* all kernel launches in the call */
+  int32_t m_tiles;            /* 128-row tiles over all experts incl. shared */
+} slp_moe_stats;
+
+/* Buffers readable through slp_moe_debug_buffer (parity / evidence; layouts in DESIGN.md §5). */
+typedef enum {
+  SLP_BUF_COUNTS = 0,      /* int32 [E] tokens per routed expert */
+  SLP_BUF_ROW_START = 1,   /* int32 [E+1] first workspace row of each expert (entry E = shared) */
+  SLP_BUF_POS = 2,         /* int32 [T, k] workspace row of (t, j) */
+  SLP_BUF_ROW_TOKEN = 3,   /* int32 [rows] token id of each workspace row (-1 = padding) */
+  SLP_BUF_HQ = 4,          /* uint8 [rows, I] requantised SwiGLU output */
+  SLP_BUF_HS = 5,          /* float [rows, ceil4(I/128)] its scales */
+  SLP_BUF_Y = 6,           /* bf16  [rows, H] per-row expert outputs */
+  SLP_BUF_LOGITS = 7       /* float [T, E] router logits */
+} slp_debug_buffer_id;
+
+/* Create a layer.  Validates shapes, pins (or checks) the host weights, uploads the resident
+ * tensors, allocates workspace for cfg->max_tokens and the expert slots.  Starts in SLP_STREAMED.
+ * Errors: INVALID_ARG (NULL / bad struct_size), UNSUPPORTED_SHAPE, NOT_PINNED, OOM, CUDA. */
+slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weights* w, slp_moe_layer** out);
+
+/* Switch residency.  SLP_RESIDENT uploads all E experts into HBM once (blocking) and later calls
+ * copy nothing; SLP_STREAMED frees that copy and returns to per-call streaming.  Blocks until the
+ * handle is idle. */
+slp_status slp_moe_set_residency(slp_moe_layer* h, slp_residency r);
+
+/* out[t,:] = sum_j w[t,j] * FFN_{idx[t,j]}(hidden[t,:]) + FFN_shared(hidden[t,:]), bf16, no residual.
+ *  hidden_bf16: dev [T, H] bf16, read only.  out_bf16: dev [T, H] bf16, fully overwritten; must
+ *  not alias hidden.  T in 0..max_tokens (T == 0 returns SLP_OK and touches nothing).
+ *  cuda_stream: a cudaStream_t (0 = legacy default stream).  Asynchronous: all work is ordered
+ *  after prior work on cuda_stream and `out` is valid for later work on it.  The library's copy
+ *  stream is joined to cuda_stream by events.  One call in flight per handle: a second call
+ *  before the first has finished on the device returns SLP_ERR_BUSY.
+ *  With skip_empty_experts == 1 the call synchronises cuda_stream once internally. */
+slp_status slp_moe_prefill(slp_moe_layer* h, const void* hidden_bf16, int32_t T, void* out_bf16, void* cuda_stream);
+
+/* End-to-end convenience: same as slp_moe_prefill but hidden/out are HOST buffers ([T,H] bf16,
+ * pinned for full speed); copies in and out through an internal device buffer on the internal
+ * compute stream and returns when `out` is complete. */
+slp_status slp_moe_prefill_host(slp_moe_layer* h, const void* hidden_bf16_host, int32_t T, void* out_bf16_host);
+
+/* Waits for the in-flight call (if any) and releases everything create allocated or pinned. */
+slp_status slp_moe_layer_destroy(slp_moe_layer* h);
+
+/* Thread-local description of the last error on this thread ("" if none). */
+const char* slp_last_error(void);
+
+/* Parity / evidence exports.  Each waits for the in-flight call, then copies device -> host. */
+slp_status slp_moe_debug_routing(slp_moe_layer* h, int32_t* idx /*[T,k]*/, float* w /*[T,k]*/, int32_t* counts /*[E]*/);
+slp_status slp_moe_debug_quant_hidden(slp_moe_layer* h, uint8_t* xq /*[T,H]*/, float* xs /*[T,H/128]*/);
+/* Copies min(bytes, size of the buffer for the last call) bytes; *written gets that size. */
+slp_status slp_moe_debug_buffer(slp_moe_layer* h, int32_t which, void* host_dst, size_t bytes, size_t* written);
+slp_status slp_moe_get_stats(slp_moe_layer* h, slp_moe_stats* stats);
+
+/* Measures pinned host -> device bandwidth on `device` with back-to-back cudaMemcpyAsync of
+ * `chunk_bytes` each (total `total_bytes`, best of `repeats`); writes GB/s (1e9) to *gbs.
+ * This is the denominator of the streamed-mode roofline. */
+slp_status slp_measure_h2d(int32_t device, size_t chunk_bytes, size_t total_bytes, int32_t repeats, double* gbs);
+
+/* Library version string. */
+const char* slp_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SLP_MOE_H */

@@ -1,7 +1,206 @@
-# placeholder, replaced below
-class SlpMoeLayer: pass
-class SlpError(Exception): pass
-def lib(): raise RuntimeError
-def library_path(): return ""
-def measure_h2d_gbs(*a, **k): raise RuntimeError
-EXPORTED_SYMBOLS = []
+"""ctypes binding of libslpmoe.so (include/slp_moe.h) — argument marshalling only.
+
+Every function here maps one-to-one onto a C-ABI entry point; no step of the path is computed in
+Python or PyTorch.  PyTorch tensors are used for device memory and streams only.  The library
+is loaded on first use; a missing build raises immediately (there is no fallback).
+"""
+
+import ctypes as C
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB = None
+
+EXPORTED_SYMBOLS = [
+    "slp_moe_layer_create", "slp_moe_set_residency", "slp_moe_prefill", "slp_moe_prefill_host",
+    "slp_moe_layer_destroy", "slp_last_error", "slp_moe_debug_routing",
+    "slp_moe_debug_quant_hidden", "slp_moe_debug_buffer", "slp_moe_get_stats",
+    "slp_measure_h2d", "slp_version",
+]
+
+SLP_STREAMED, SLP_RESIDENT = 0, 1
+SCORING = {"sigmoid_bias": 0, "softmax": 1}
+BUF = dict(counts=0, row_start=1, pos=2, row_token=3, hq=4, hs=5, y=6, logits=7)
+
+
+class SlpError(RuntimeError):
+    def __init__(self, status, message):
+        super().__init__(f"slp status {status}: {message}")
+        self.status = status
+
+
+class _Cfg(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("device", C.c_int32), ("hidden", C.c_int32),
+                ("n_experts", C.c_int32), ("top_k", C.c_int32), ("n_group", C.c_int32),
+                ("topk_group", C.c_int32), ("moe_intermediate", C.c_int32),
+                ("n_shared", C.c_int32), ("shared_intermediate", C.c_int32),
+                ("scoring", C.c_int32), ("norm_topk", C.c_int32), ("routed_scale", C.c_float),
+                ("max_tokens", C.c_int32), ("staging_slots", C.c_int32),
+                ("experts_per_launch", C.c_int32), ("skip_empty_experts", C.c_int32),
+                ("require_pinned", C.c_int32), ("gemm_impl", C.c_int32)]
+
+
+class _HostWeights(C.Structure):
+    _fields_ = [("router_w", C.c_void_p), ("router_bias", C.c_void_p),
+                ("gate_q", C.POINTER(C.c_void_p)), ("gate_s", C.POINTER(C.c_void_p)),
+                ("up_q", C.POINTER(C.c_void_p)), ("up_s", C.POINTER(C.c_void_p)),
+                ("down_q", C.POINTER(C.c_void_p)), ("down_s", C.POINTER(C.c_void_p)),
+                ("shared_gate_q", C.c_void_p), ("shared_gate_s", C.c_void_p),
+                ("shared_up_q", C.c_void_p), ("shared_up_s", C.c_void_p),
+                ("shared_down_q", C.c_void_p), ("shared_down_s", C.c_void_p)]
+
+
+class Stats(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("tokens", C.c_int32), ("residency", C.c_int32),
+                ("experts_copied", C.c_int32), ("experts_skipped", C.c_int32),
+                ("bytes_copied", C.c_int64), ("ms_total", C.c_float), ("ms_copy_span", C.c_float),
+                ("ms_route", C.c_float), ("ms_experts", C.c_float), ("ms_combine", C.c_float),
+                ("gemm_launches", C.c_int32), ("kernel_launches", C.c_int32), ("m_tiles", C.c_int32)]
+
+    def as_dict(self):
+        return {n: getattr(self, n) for n, _ in self._fields_ if n != "struct_size"}
+
+
+def library_path():
+    return os.path.join(_HERE, "libslpmoe.so")
+
+
+def lib():
+    """Loads libslpmoe.so (once).  Raises if it has not been built."""
+    global _LIB
+    if _LIB is None:
+        path = library_path()
+        if not os.path.exists(path):
+            raise ImportError(f"{path} not found: build it with `python __graft_entry__.py` "
+                              "(the SLP MoE path has no fallback implementation)")
+        L = C.CDLL(path)
+        L.slp_last_error.restype = C.c_char_p
+        L.slp_version.restype = C.c_char_p
+        L.slp_moe_layer_create.argtypes = [C.POINTER(_Cfg), C.POINTER(_HostWeights), C.POINTER(C.c_void_p)]
+        L.slp_moe_set_residency.argtypes = [C.c_void_p, C.c_int]
+        L.slp_moe_prefill.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
+        L.slp_moe_prefill_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
+        L.slp_moe_layer_destroy.argtypes = [C.c_void_p]
+        L.slp_moe_debug_routing.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.slp_moe_debug_quant_hidden.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.slp_moe_debug_buffer.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_size_t, C.POINTER(C.c_size_t)]
+        L.slp_moe_get_stats.argtypes = [C.c_void_p, C.POINTER(Stats)]
+        L.slp_measure_h2d.argtypes = [C.c_int32, C.c_size_t, C.c_size_t, C.c_int32, C.POINTER(C.c_double)]
+        for name in EXPORTED_SYMBOLS:
+            if name not in ("slp_last_error", "slp_version"):
+                getattr(L, name).restype = C.c_int
+        _LIB = L
+    return _LIB
+
+
+def _check(status):
+    if status != 0:
+        raise SlpError(status, lib().slp_last_error().decode())
+
+
+def measure_h2d_gbs(device=0, chunk_bytes=44040192, total_bytes=1 << 30, repeats=5):
+    out = C.c_double(0)
+    _check(lib().slp_measure_h2d(device, chunk_bytes, total_bytes, repeats, C.byref(out)))
+    return out.value
+
+
+def _ptr_array(tensor):
+    """E pointers to the per-expert slices of a host tensor with leading expert axis."""
+    n = tensor.shape[0]
+    arr = (C.c_void_p * n)()
+    for e in range(n):
+        arr[e] = tensor[e].data_ptr()
+    return arr
+
+
+class SlpMoeLayer:
+    """One MoE layer handle.  `weights` is the dict `inputs.make_weights` returns (host torch
+    tensors, kept alive by this object because the library borrows the memory)."""
+
+    def __init__(self, cfg, weights, *, max_tokens=None, device=0, staging_slots=0,
+                 experts_per_launch=0, skip_empty_experts=False, require_pinned=False, gemm_impl=0):
+        self._h = C.c_void_p()
+        self.cfg = cfg
+        self.weights = weights
+        self.max_tokens = max_tokens or cfg.T
+        c = _Cfg(struct_size=C.sizeof(_Cfg), device=device, hidden=cfg.H, n_experts=cfg.E,
+                 top_k=cfg.k, n_group=cfg.G, topk_group=cfg.Gk, moe_intermediate=cfg.I,
+                 n_shared=cfg.n_shared, shared_intermediate=cfg.I if cfg.n_shared else 0,
+                 scoring=SCORING[cfg.scoring], norm_topk=int(cfg.norm_topk),
+                 routed_scale=cfg.routed_scale, max_tokens=self.max_tokens,
+                 staging_slots=staging_slots, experts_per_launch=experts_per_launch,
+                 skip_empty_experts=int(skip_empty_experts), require_pinned=int(require_pinned),
+                 gemm_impl=gemm_impl)
+        w = weights
+        self._arrays = {k: _ptr_array(w[k]) for k in ("gate_q", "gate_s", "up_q", "up_s", "down_q", "down_s")}
+
+        def p(t):
+            return None if t is None else t.data_ptr()
+
+        hw = _HostWeights(router_w=p(w["router_w"]), router_bias=p(w["router_bias"]),
+                          shared_gate_q=p(w["shared_gate_q"]), shared_gate_s=p(w["shared_gate_s"]),
+                          shared_up_q=p(w["shared_up_q"]), shared_up_s=p(w["shared_up_s"]),
+                          shared_down_q=p(w["shared_down_q"]), shared_down_s=p(w["shared_down_s"]))
+        for k, arr in self._arrays.items():
+            setattr(hw, k, C.cast(arr, C.POINTER(C.c_void_p)))
+        _check(lib().slp_moe_layer_create(C.byref(c), C.byref(hw), C.byref(self._h)))
+
+    # -- the C-ABI calls ------------------------------------------------------------------
+    def set_residency(self, mode):
+        r = {"streamed": SLP_STREAMED, "resident": SLP_RESIDENT}[mode]
+        _check(lib().slp_moe_set_residency(self._h, r))
+
+    def prefill(self, hidden, out=None, stream=None):
+        """hidden: CUDA bf16 [T, H] tensor.  Asynchronous on `stream` (default: current)."""
+        import torch
+        assert hidden.is_cuda and hidden.dtype == torch.bfloat16 and hidden.is_contiguous()
+        if out is None:
+            out = torch.empty_like(hidden)
+        s = torch.cuda.current_stream(hidden.device) if stream is None else stream
+        _check(lib().slp_moe_prefill(self._h, hidden.data_ptr(), hidden.shape[0], out.data_ptr(), s.cuda_stream))
+        return out
+
+    def prefill_host(self, hidden_host, out_host):
+        """hidden_host/out_host: HOST bf16 [T, H] tensors (pinned for full speed).  Blocking."""
+        _check(lib().slp_moe_prefill_host(self._h, hidden_host.data_ptr(), hidden_host.shape[0], out_host.data_ptr()))
+        return out_host
+
+    def debug_routing(self, T):
+        import numpy as np
+        idx = np.empty((T, self.cfg.k), np.int32)
+        w = np.empty((T, self.cfg.k), np.float32)
+        counts = np.empty(self.cfg.E, np.int32)
+        _check(lib().slp_moe_debug_routing(self._h, idx.ctypes.data, w.ctypes.data, counts.ctypes.data))
+        return idx, w, counts
+
+    def debug_quant_hidden(self, T):
+        import numpy as np
+        xq = np.empty((T, self.cfg.H), np.uint8)
+        xs = np.empty((T, self.cfg.H // 128), np.float32)
+        _check(lib().slp_moe_debug_quant_hidden(self._h, xq.ctypes.data, xs.ctypes.data))
+        return xq, xs
+
+    def debug_buffer(self, name, dtype):
+        import numpy as np
+        size = C.c_size_t(0)
+        probe = np.empty(1, np.uint8)
+        _check(lib().slp_moe_debug_buffer(self._h, BUF[name], probe.ctypes.data, 0, C.byref(size)))
+        buf = np.empty(size.value, np.uint8)
+        _check(lib().slp_moe_debug_buffer(self._h, BUF[name], buf.ctypes.data, size.value, C.byref(size)))
+        return buf.view(dtype)
+
+    def stats(self):
+        st = Stats(struct_size=C.sizeof(Stats))
+        _check(lib().slp_moe_get_stats(self._h, C.byref(st)))
+        return st.as_dict()
+
+    def close(self):
+        if self._h:
+            lib().slp_moe_layer_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

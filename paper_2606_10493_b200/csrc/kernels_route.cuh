@@ -1,0 +1,401 @@
+// kernels_route.cuh — router (a1), histogram/scan/permute (a2), hidden quantisation (a3) and the
+// weighted combine (a9) of the SLP MoE layer.  See DESIGN.md §6 for the per-kernel rooflines.
+#pragma once
+#include <cstdint>
+#include <cuda_bf16.h>
+#include <cuda_fp8.h>
+
+namespace slp {
+
+constexpr int kBlock = 128;        // scale-block length
+constexpr int kChunkTokens = 128;  // tokens one warp ranks in the permute kernels
+constexpr int kMaxExperts = 512;
+
+__device__ __forceinline__ float bf16_bits_to_float(uint16_t b) { return __uint_as_float(static_cast<uint32_t>(b) << 16); }
+
+// ---------------------------------------------------------------------------------------------
+// a1 (first half): router logits[t, e] = sum_h x[t, h] * W_r[e, h], fp32 FMA, fp32 accumulate.
+// x is bf16 (exact in fp32).  64x64 output tile per block, 16-deep K steps, 4x4 per thread.
+// ("A learned gating mechanism selects ... top-k or grouped top-k".)
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) router_logits_kernel(const uint16_t* __restrict__ x, const float* __restrict__ w,
+                                                            float* __restrict__ logits, int T, int H, int E) {
+  constexpr int BM = 64, BN = 64, BK = 16;
+  __shared__ float As[BK][BM + 4];
+  __shared__ float Bs[BK][BN + 4];
+  const int t0 = blockIdx.x * BM, e0 = blockIdx.y * BN;
+  const int tid = threadIdx.x, tx = tid % 16, ty = tid / 16;
+  float acc[4][4] = {};
+  const int lr = tid / 4, lc = (tid % 4) * 4;  // loader: row 0..63, 4 consecutive k
+  for (int k0 = 0; k0 < H; k0 += BK) {
+    {
+      int t = t0 + lr;
+      float v[4] = {0, 0, 0, 0};
+      if (t < T) {
+        uint2 raw = *reinterpret_cast<const uint2*>(x + static_cast<size_t>(t) * H + k0 + lc);
+        v[0] = bf16_bits_to_float(raw.x & 0xFFFF); v[1] = bf16_bits_to_float(raw.x >> 16);
+        v[2] = bf16_bits_to_float(raw.y & 0xFFFF); v[3] = bf16_bits_to_float(raw.y >> 16);
+      }
+#pragma unroll
+      for (int i = 0; i < 4; ++i) As[lc + i][lr] = v[i];
+      int e = e0 + lr;
+      float4 wv = make_float4(0, 0, 0, 0);
+      if (e < E) wv = *reinterpret_cast<const float4*>(w + static_cast<size_t>(e) * H + k0 + lc);
+      Bs[lc + 0][lr] = wv.x; Bs[lc + 1][lr] = wv.y; Bs[lc + 2][lr] = wv.z; Bs[lc + 3][lr] = wv.w;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int kk = 0; kk < BK; ++kk) {
+      float a[4], b[4];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) a[i] = As[kk][ty * 4 + i];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) b[j] = Bs[kk][tx * 4 + j];
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j] = fmaf(a[i], b[j], acc[i][j]);
+    }
+    __syncthreads();
+  }
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    int t = t0 + ty * 4 + i;
+    if (t >= T) continue;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      int e = e0 + tx * 4 + j;
+      if (e < E) logits[static_cast<size_t>(t) * E + e] = acc[i][j];
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a1 (second half): scores, group-limited selection and weights; one warp per token.
+// Lane l holds experts l, l+32, ...  Ties go to the lower index (Q3).
+//   sigmoid_bias: s = sigmoid(logit), sel = s + bias; groups scored by their two best sel;
+//                 topk_group best groups kept, the rest excluded; top_k best sel among kept;
+//                 w_j = s_j (/ sum) * scale.
+//   softmax:      selection by logit (monotone in p); w_j = exp(l_j - max) / Z, with Z the sum
+//                 over the selected (norm_topk) or over all experts.
+// ---------------------------------------------------------------------------------------------
+struct ArgMax {
+  float v;
+  int i;
+};
+__device__ __forceinline__ ArgMax warp_argmax(float v, int i) {
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) {
+    float ov = __shfl_xor_sync(0xFFFFFFFFu, v, off);
+    int oi = __shfl_xor_sync(0xFFFFFFFFu, i, off);
+    if (ov > v || (ov == v && oi < i)) { v = ov; i = oi; }
+  }
+  return {v, i};
+}
+
+template <int kPerLane>
+__global__ void __launch_bounds__(256) router_topk_kernel(const float* __restrict__ logits, const float* __restrict__ bias,
+                                                          int32_t* __restrict__ idx, float* __restrict__ wout, int T, int E,
+                                                          int k, int G, int Gk, int scoring, int norm_topk, float scale) {
+  const int lane = threadIdx.x & 31;
+  const int t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (t >= T) return;
+  const float NEG = -INFINITY;
+  float s[kPerLane], sel[kPerLane];
+  float lmax = NEG;
+#pragma unroll
+  for (int r = 0; r < kPerLane; ++r) {
+    int e = lane + 32 * r;
+    float l = (e < E) ? logits[static_cast<size_t>(t) * E + e] : NEG;
+    s[r] = l;
+    lmax = fmaxf(lmax, l);
+  }
+  if (scoring == 0) {
+#pragma unroll
+    for (int r = 0; r < kPerLane; ++r) {
+      int e = lane + 32 * r;
+      if (e < E) {
+        float sc = 1.0f / (1.0f + expf(-s[r]));
+        s[r] = sc;
+        sel[r] = sc + (bias ? bias[e] : 0.0f);
+      } else {
+        sel[r] = NEG;
+      }
+    }
+  } else {
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) lmax = fmaxf(lmax, __shfl_xor_sync(0xFFFFFFFFu, lmax, off));
+    float z = 0.f;
+#pragma unroll
+    for (int r = 0; r < kPerLane; ++r) {
+      int e = lane + 32 * r;
+      sel[r] = (e < E) ? s[r] : NEG;             // select by logit
+      s[r] = (e < E) ? expf(s[r] - lmax) : 0.f;  // unnormalised probability
+      z += s[r];
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) z += __shfl_xor_sync(0xFFFFFFFFu, z, off);
+    if (!norm_topk) {
+      float inv = 1.0f / z;
+#pragma unroll
+      for (int r = 0; r < kPerLane; ++r) s[r] *= inv;
+    }
+  }
+
+  if (G > 1) {
+    const int gs = E / G;
+    float my_gscore = NEG;  // lane g (< G) keeps group g's score; G <= 32 checked at create
+    for (int g = 0; g < G; ++g) {
+      float m1 = NEG, m2 = NEG;
+#pragma unroll
+      for (int r = 0; r < kPerLane; ++r) {
+        int e = lane + 32 * r;
+        if (e < E && e / gs == g) {
+          float v = sel[r];
+          if (v > m1) { m2 = m1; m1 = v; } else if (v > m2) { m2 = v; }
+        }
+      }
+#pragma unroll
+      for (int off = 16; off > 0; off >>= 1) {
+        float o1 = __shfl_xor_sync(0xFFFFFFFFu, m1, off);
+        float o2 = __shfl_xor_sync(0xFFFFFFFFu, m2, off);
+        float n1 = fmaxf(m1, o1);
+        float n2 = fmaxf(fminf(m1, o1), fmaxf(m2, o2));
+        m1 = n1; m2 = n2;
+      }
+      float gsc = (gs >= 2) ? (m1 + m2) : m1;
+      if (lane == g) my_gscore = gsc;
+    }
+    uint32_t keep = 0;
+    for (int i = 0; i < Gk; ++i) {
+      ArgMax a = warp_argmax(my_gscore, lane);
+      keep |= 1u << a.i;
+      if (lane == a.i) my_gscore = NEG;
+    }
+#pragma unroll
+    for (int r = 0; r < kPerLane; ++r) {
+      int e = lane + 32 * r;
+      if (e < E && !((keep >> (e / gs)) & 1u)) sel[r] = NEG;
+    }
+  }
+
+  float my_w = 0.f;
+  int my_e = 0;
+  float wsum = 0.f;
+  for (int j = 0; j < k; ++j) {
+    float bv = NEG;
+    int bi = 0x7FFFFFFF;
+#pragma unroll
+    for (int r = 0; r < kPerLane; ++r) {
+      int e = lane + 32 * r;
+      if (e < E && (sel[r] > bv || (sel[r] == bv && e < bi))) { bv = sel[r]; bi = e; }
+    }
+    ArgMax a = warp_argmax(bv, bi);
+    float sc = 0.f;
+#pragma unroll
+    for (int r = 0; r < kPerLane; ++r) {
+      int e = lane + 32 * r;
+      if (e == a.i) { sc = s[r]; sel[r] = NEG; }
+    }
+    sc = __shfl_sync(0xFFFFFFFFu, sc, a.i & 31);
+    wsum += sc;
+    if (lane == j) { my_w = sc; my_e = a.i; }
+  }
+  if (lane < k) {
+    float wv = norm_topk ? my_w / wsum : my_w;
+    idx[static_cast<size_t>(t) * k + lane] = my_e;
+    wout[static_cast<size_t>(t) * k + lane] = wv * scale;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a2: histogram / scan / permute.  Workspace rows: [0, Tpad) hold the un-permuted tokens (the
+// shared expert's rows), then each routed expert owns a 128-aligned row range holding its tokens
+// in ascending token id ("sorted to form per-expert token lists").
+//   pass 1: per-chunk (128 tokens, one warp) expert histograms
+//   pass 2: one block: per-expert exclusive scan over chunks, counts, padded row_start,
+//           tile_start and the tile -> expert table
+//   pass 3: per chunk, stable ranks via match_any -> pos[t, j], row_token[row]
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) permute_hist_kernel(const int32_t* __restrict__ idx, int32_t* __restrict__ chunk_counts,
+                                                           int T, int k, int E) {
+  extern __shared__ int32_t sm_hist[];  // [warps][E]
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int chunk = blockIdx.x * (blockDim.x >> 5) + warp;
+  int32_t* h = sm_hist + warp * E;
+  for (int e = lane; e < E; e += 32) h[e] = 0;
+  __syncwarp();
+  const int t0 = chunk * kChunkTokens;
+  const int n = max(0, min(kChunkTokens, T - t0)) * k;
+  const int32_t* src = idx + static_cast<size_t>(t0) * k;
+  for (int i = lane; i < n; i += 32) atomicAdd(&h[src[i]], 1);
+  __syncwarp();
+  if (t0 < T)
+    for (int e = lane; e < E; e += 32) chunk_counts[static_cast<size_t>(chunk) * E + e] = h[e];
+}
+
+__global__ void __launch_bounds__(512) permute_scan_kernel(int32_t* __restrict__ chunk_counts, int32_t* __restrict__ counts,
+                                                           int32_t* __restrict__ row_start, int32_t* __restrict__ tile_start,
+                                                           int32_t* __restrict__ tile_expert, int n_chunks, int T, int E,
+                                                           int has_shared) {
+  __shared__ int32_t s_cnt[kMaxExperts + 1];
+  __shared__ int32_t s_tile[kMaxExperts + 2];
+  const int e = threadIdx.x;
+  if (e < E) {
+    int run = 0;
+    for (int c0 = 0; c0 < n_chunks; c0 += 8) {  // 8 independent loads in flight, then the serial scan
+      int v[8];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) v[u] = (c0 + u < n_chunks) ? chunk_counts[static_cast<size_t>(c0 + u) * E + e] : 0;
+#pragma unroll
+      for (int u = 0; u < 8; ++u) {
+        if (c0 + u < n_chunks) chunk_counts[static_cast<size_t>(c0 + u) * E + e] = run;
+        run += v[u];
+      }
+    }
+    s_cnt[e] = run;
+    counts[e] = run;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    const int Tpad = (T + 127) / 128 * 128;
+    int row = Tpad, tile = 0;
+    for (int i = 0; i < E; ++i) {
+      row_start[i] = row;
+      s_tile[i] = tile;
+      int mt = (s_cnt[i] + 127) / 128;
+      row += mt * 128;
+      tile += mt;
+    }
+    row_start[E] = 0;  // shared expert: the un-permuted rows
+    s_tile[E] = tile;
+    tile += has_shared ? Tpad / 128 : 0;
+    s_tile[E + 1] = tile;
+    row_start[E + 1] = row;  // total rows in use
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < E + 2; i += blockDim.x) tile_start[i] = s_tile[i];
+  for (int i = threadIdx.x; i <= E; i += blockDim.x)
+    for (int m = s_tile[i]; m < s_tile[i + 1]; ++m) tile_expert[m] = i;
+}
+
+__global__ void __launch_bounds__(128) permute_place_kernel(const int32_t* __restrict__ idx, const int32_t* __restrict__ chunk_off,
+                                                            const int32_t* __restrict__ row_start, int32_t* __restrict__ pos,
+                                                            int32_t* __restrict__ row_token, int T, int k, int E) {
+  extern __shared__ int32_t sm_run[];  // [warps][E] next free row of each expert for this chunk
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int chunk = blockIdx.x * (blockDim.x >> 5) + warp;
+  const int t0 = chunk * kChunkTokens;
+  if (t0 >= T) return;
+  int32_t* run = sm_run + warp * E;
+  for (int e = lane; e < E; e += 32) run[e] = row_start[e] + chunk_off[static_cast<size_t>(chunk) * E + e];
+  __syncwarp();
+  const int n = min(kChunkTokens, T - t0) * k;
+  const int32_t* src = idx + static_cast<size_t>(t0) * k;
+  for (int base = 0; base < n; base += 32) {
+    const int i = base + lane;
+    const bool valid = i < n;
+    const int e = valid ? src[i] : -1 - lane;  // entries are token-major: ascending lane = ascending token
+    const uint32_t peers = __match_any_sync(0xFFFFFFFFu, e);
+    const int rank = __popc(peers & ((1u << lane) - 1));
+    int dst = 0;
+    if (valid) dst = run[e] + rank;
+    __syncwarp();
+    if (valid && rank == 0) run[e] += __popc(peers);
+    __syncwarp();
+    if (valid) {
+      const int t = t0 + i / k;
+      pos[static_cast<size_t>(t0) * k + i] = dst;
+      row_token[dst] = t;
+    }
+  }
+  for (int i = lane; i < min(kChunkTokens, T - t0); i += 32) row_token[t0 + i] = t0 + i;  // shared rows
+}
+
+// ---------------------------------------------------------------------------------------------
+// a3: hidden quantisation, fused with the scatter into expert order.  Per token, per 128
+// channels: amax -> s = amax / 448 -> e4m3(x / s) (fp32 IEEE division, RNE, saturating), written
+// to the token's own row (shared-expert region) and to its k expert rows.
+// ("activations are quantized to FP8"; Q10-Q12.)
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t quant4_e4m3(float a, float b, float c, float d, float s) {
+  __nv_fp8x2_storage_t lo = __nv_cvt_float2_to_fp8x2(make_float2(__fdiv_rn(a, s), __fdiv_rn(b, s)), __NV_SATFINITE, __NV_E4M3);
+  __nv_fp8x2_storage_t hi = __nv_cvt_float2_to_fp8x2(make_float2(__fdiv_rn(c, s), __fdiv_rn(d, s)), __NV_SATFINITE, __NV_E4M3);
+  return static_cast<uint32_t>(lo) | (static_cast<uint32_t>(hi) << 16);
+}
+
+__global__ void __launch_bounds__(256) quant_scatter_kernel(const uint16_t* __restrict__ x, const int32_t* __restrict__ pos,
+                                                            uint8_t* __restrict__ xq, float* __restrict__ xs, int T, int H, int k,
+                                                            int xs_stride) {
+  const int t = blockIdx.x;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
+  __shared__ int32_t dst[33];
+  if (threadIdx.x < k) dst[threadIdx.x + 1] = pos[static_cast<size_t>(t) * k + threadIdx.x];
+  if (threadIdx.x == 0) dst[0] = t;
+  __syncthreads();
+  const int nkb = H / kBlock;
+  for (int kb = warp; kb < nkb; kb += nwarps) {
+    const uint2 raw = *reinterpret_cast<const uint2*>(x + static_cast<size_t>(t) * H + kb * kBlock + lane * 4);
+    const float a = bf16_bits_to_float(raw.x & 0xFFFF), b = bf16_bits_to_float(raw.x >> 16);
+    const float c = bf16_bits_to_float(raw.y & 0xFFFF), d = bf16_bits_to_float(raw.y >> 16);
+    float amax = fmaxf(fmaxf(fabsf(a), fabsf(b)), fmaxf(fabsf(c), fabsf(d)));
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xFFFFFFFFu, amax, off));
+    const float s = (amax == 0.f) ? 1.0f : __fdiv_rn(amax, 448.0f);
+    const uint32_t q = quant4_e4m3(a, b, c, d, s);
+    for (int j = 0; j <= k; ++j) {
+      const size_t row = dst[j];
+      *reinterpret_cast<uint32_t*>(xq + row * H + kb * kBlock + lane * 4) = q;
+      if (lane == 0) xs[row * xs_stride + kb] = s;
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a9: weighted combine.  out[t] = sum_j w[t,j] * Y[pos[t,j]] (fixed j order, fp32 FMA) + Y[t]
+// (shared expert row, weight 1), rounded once to bf16.  Gather-based, no atomics.
+// (PAPER.md:92 step 5 "A final weighted sum"; "router-weighted accumulation in F32".)
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) combine_kernel(const __nv_bfloat16* __restrict__ y, const int32_t* __restrict__ pos,
+                                                      const float* __restrict__ w, __nv_bfloat16* __restrict__ out, int T, int H,
+                                                      int k, int has_shared) {
+  const int t = blockIdx.x;
+  __shared__ int32_t s_row[32];
+  __shared__ float s_w[32];
+  if (threadIdx.x < k) {
+    s_row[threadIdx.x] = pos[static_cast<size_t>(t) * k + threadIdx.x];
+    s_w[threadIdx.x] = w[static_cast<size_t>(t) * k + threadIdx.x];
+  }
+  __syncthreads();
+  for (int c = threadIdx.x * 8; c < H; c += blockDim.x * 8) {
+    float acc[8] = {};
+    for (int j = 0; j < k; ++j) {
+      const uint4 raw = *reinterpret_cast<const uint4*>(y + static_cast<size_t>(s_row[j]) * H + c);
+      const uint32_t r[4] = {raw.x, raw.y, raw.z, raw.w};
+      const float wj = s_w[j];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        acc[2 * i] = fmaf(wj, __uint_as_float(r[i] << 16), acc[2 * i]);
+        acc[2 * i + 1] = fmaf(wj, __uint_as_float(r[i] & 0xFFFF0000u), acc[2 * i + 1]);
+      }
+    }
+    if (has_shared) {
+      const uint4 raw = *reinterpret_cast<const uint4*>(y + static_cast<size_t>(t) * H + c);
+      const uint32_t r[4] = {raw.x, raw.y, raw.z, raw.w};
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        acc[2 * i] += __uint_as_float(r[i] << 16);
+        acc[2 * i + 1] += __uint_as_float(r[i] & 0xFFFF0000u);
+      }
+    }
+    uint32_t o[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      __nv_bfloat162 p = __floats2bfloat162_rn(acc[2 * i], acc[2 * i + 1]);
+      o[i] = *reinterpret_cast<uint32_t*>(&p);
+    }
+    *reinterpret_cast<uint4*>(out + static_cast<size_t>(t) * H + c) = make_uint4(o[0], o[1], o[2], o[3]);
+  }
+}
+
+}  // namespace slp

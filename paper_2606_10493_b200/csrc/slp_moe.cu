@@ -1,0 +1,765 @@
+// slp_moe.cu — host side of libslpmoe: handle, C ABI (include/slp_moe.h), workspace, TMA
+// descriptors and the streaming engine (a4) that overlaps host->HBM expert-weight copies with the
+// grouped GEMMs (Fig. 5: loader / model / unloader with ON / OFF events and an
+// experts ring buffer).  On one device the three roles collapse to two CUDA streams and two event
+// arrays: the copy stream is the loader, the caller's stream is the model thread, and "unload" is
+// the slot-free event the loader waits on before it overwrites a ring slot (the authoritative copy
+// stays on the host, so nothing is copied back).
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/slp_moe.h"
+#include "kernels_gemm_simt.cuh"
+#include "kernels_gemm_tc.cuh"
+#include "kernels_route.cuh"
+
+namespace {
+
+thread_local std::string g_last_error;
+
+slp_status fail(slp_status st, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  g_last_error = buf;
+  return st;
+}
+
+#define CU_TRY(expr)                                                                                   \
+  do {                                                                                                 \
+    cudaError_t _e = (expr);                                                                           \
+    if (_e != cudaSuccess) {                                                                           \
+      slp_status _st = (_e == cudaErrorMemoryAllocation) ? SLP_ERR_OOM : SLP_ERR_CUDA;                 \
+      return fail(_st, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(_e), __FILE__, __LINE__);    \
+    }                                                                                                  \
+  } while (0)
+
+using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  static std::once_flag once;
+  std::call_once(once, [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeTiledFn>(p);
+  });
+  return fn;
+}
+
+// 2D uint8 tensor [rows, inner] (row stride = inner bytes), box 128 B x 128 rows, 128B swizzle.
+slp_status make_tmap_u8(CUtensorMap* tm, void* base, uint64_t inner, uint64_t rows) {
+  EncodeTiledFn fn = get_encode_fn();
+  if (!fn) return fail(SLP_ERR_CUDA, "cuTensorMapEncodeTiled not available from the driver");
+  cuuint64_t dims[2] = {inner, rows};
+  cuuint64_t strides[1] = {inner};
+  cuuint32_t box[2] = {128, 128};
+  cuuint32_t estr[2] = {1, 1};
+  CUresult r = fn(tm, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                  CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(SLP_ERR_CUDA, "cuTensorMapEncodeTiled failed with CUresult %d", static_cast<int>(r));
+  return SLP_OK;
+}
+
+inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
+
+}  // namespace
+
+struct slp_moe_layer {
+  slp_moe_cfg cfg{};
+  slp_moe_host_weights hw{};
+  std::vector<const uint8_t*> gate_q, up_q, down_q;
+  std::vector<void*> registered;  // host ranges pinned by create
+  int H = 0, E = 0, k = 0, I = 0, Tm = 0;
+  int kbH = 0, kbI = 0, xs_stride = 0, hs_stride = 0;
+  int rows_max = 0, tiles_max = 0, n_chunks_max = 0;
+  int num_sms = 0;
+  size_t slot_bytes = 0;
+  int n_stage = 0;       // routed-expert slots currently in the pool (E when resident)
+  int epl = 0;           // experts per launch (streamed)
+  int residency = SLP_STREAMED;
+
+  // resident device tensors
+  float *d_router_w = nullptr, *d_bias = nullptr, *d_gate_s = nullptr, *d_up_s = nullptr, *d_down_s = nullptr;
+  uint8_t* d_pool = nullptr;  // [1 + n_stage] slots; slot 0 = shared expert
+  // workspace
+  float *d_logits = nullptr, *d_w = nullptr, *d_xs = nullptr, *d_hs = nullptr;
+  int32_t *d_idx = nullptr, *d_counts = nullptr, *d_chunk = nullptr, *d_row_start = nullptr, *d_tile_start = nullptr,
+          *d_tile_expert = nullptr, *d_pos = nullptr, *d_row_token = nullptr;
+  uint8_t *d_xq = nullptr, *d_hq = nullptr;
+  __nv_bfloat16* d_y = nullptr;
+  int* d_err = nullptr;
+  void *d_e2e_in = nullptr, *d_e2e_out = nullptr;
+  int32_t* h_counts = nullptr;  // pinned
+  int* h_err = nullptr;         // pinned
+
+  CUtensorMap tm_xq{}, tm_hq{}, tm_wgu{}, tm_wd{};
+
+  cudaStream_t copy_stream = nullptr, own_stream = nullptr;
+  std::vector<cudaEvent_t> ev_ready, ev_free;
+  std::vector<char> free_recorded;
+  cudaEvent_t ev_done = nullptr, ev_t[6] = {}, ev_copy0 = nullptr, ev_copy1 = nullptr;
+  bool in_flight = false;
+  cudaStream_t last_stream = nullptr;
+  int last_T = 0;
+  slp_moe_stats stats{};
+  bool stats_copy_valid = false;
+};
+
+namespace {
+
+using L = slp_moe_layer;
+
+void free_pool(L* h) {
+  if (h->d_pool) cudaFree(h->d_pool);
+  h->d_pool = nullptr;
+  for (auto e : h->ev_ready) cudaEventDestroy(e);
+  for (auto e : h->ev_free) cudaEventDestroy(e);
+  h->ev_ready.clear();
+  h->ev_free.clear();
+  h->free_recorded.clear();
+}
+
+// (Re)allocates the expert pool with `n_stage` routed slots (+ slot 0 for the shared expert),
+// uploads the shared expert, rebuilds the weight tensor maps and the ring events.
+slp_status alloc_pool(L* h, int n_stage, int epl) {
+  free_pool(h);
+  h->n_stage = n_stage;
+  h->epl = epl;
+  const size_t bytes = static_cast<size_t>(1 + n_stage) * h->slot_bytes;
+  CU_TRY(cudaMalloc(&h->d_pool, bytes));
+  const size_t IH = static_cast<size_t>(h->I) * h->H;
+  if (h->cfg.n_shared) {
+    CU_TRY(cudaMemcpy(h->d_pool, h->hw.shared_gate_q, IH, cudaMemcpyHostToDevice));
+    CU_TRY(cudaMemcpy(h->d_pool + IH, h->hw.shared_up_q, IH, cudaMemcpyHostToDevice));
+    CU_TRY(cudaMemcpy(h->d_pool + 2 * IH, h->hw.shared_down_q, IH, cudaMemcpyHostToDevice));
+  } else {
+    CU_TRY(cudaMemset(h->d_pool, 0, h->slot_bytes));
+  }
+  slp_status st = make_tmap_u8(&h->tm_wgu, h->d_pool, h->H, static_cast<uint64_t>(1 + n_stage) * 3 * h->I);
+  if (st != SLP_OK) return st;
+  st = make_tmap_u8(&h->tm_wd, h->d_pool, h->I, static_cast<uint64_t>(1 + n_stage) * 3 * h->H);
+  if (st != SLP_OK) return st;
+  const int n_groups = (n_stage + epl - 1) / epl;
+  h->ev_ready.resize(n_groups);
+  h->ev_free.resize(n_groups);
+  h->free_recorded.assign(n_groups, 0);
+  for (int i = 0; i < n_groups; ++i) {
+    CU_TRY(cudaEventCreateWithFlags(&h->ev_ready[i], cudaEventDisableTiming));
+    CU_TRY(cudaEventCreateWithFlags(&h->ev_free[i], cudaEventDisableTiming));
+  }
+  return SLP_OK;
+}
+
+slp_status pin_range(L* h, const void* p, size_t bytes, const char* what) {
+  cudaPointerAttributes attr{};
+  cudaError_t e = cudaPointerGetAttributes(&attr, p);
+  if (e == cudaSuccess && (attr.type == cudaMemoryTypeHost || attr.type == cudaMemoryTypeManaged)) return SLP_OK;
+  cudaGetLastError();
+  if (h->cfg.require_pinned) return fail(SLP_ERR_NOT_PINNED, "%s is pageable host memory and require_pinned is set", what);
+  e = cudaHostRegister(const_cast<void*>(p), bytes, cudaHostRegisterDefault);
+  if (e == cudaErrorHostMemoryAlreadyRegistered) {
+    cudaGetLastError();
+    return SLP_OK;
+  }
+  if (e != cudaSuccess) return fail(SLP_ERR_NOT_PINNED, "cudaHostRegister(%s, %zu bytes) failed: %s", what, bytes, cudaGetErrorString(e));
+  h->registered.push_back(const_cast<void*>(p));
+  return SLP_OK;
+}
+
+slp_status wait_idle(L* h) {
+  if (h->in_flight) {
+    CU_TRY(cudaEventSynchronize(h->ev_done));
+    h->in_flight = false;
+  }
+  return SLP_OK;
+}
+
+slp_status check_kernel_error(L* h) {
+  if (*h->h_err != 0) {
+    int code = *h->h_err;
+    *h->h_err = 0;
+    cudaMemset(h->d_err, 0, sizeof(int));
+    return fail(SLP_ERR_KERNEL_TIMEOUT, "grouped GEMM pipeline wait timed out (role code %d)", code);
+  }
+  return SLP_OK;
+}
+
+slp::GemmArgs gemm_args(L* h, int mode, int e_begin, int e_end, int T) {
+  slp::GemmArgs g{};
+  g.tile_expert = h->d_tile_expert;
+  g.tile_start = h->d_tile_start;
+  g.row_start = h->d_row_start;
+  g.counts = h->d_counts;
+  g.e_begin = e_begin;
+  g.e_end = e_end;
+  g.E = h->E;
+  g.T = T;
+  g.n_stage = h->n_stage;
+  g.a_q = mode == 0 ? h->d_xq : h->d_hq;
+  g.a_s = mode == 0 ? h->d_xs : h->d_hs;
+  g.a_s_stride = mode == 0 ? h->xs_stride : h->hs_stride;
+  g.pool = h->d_pool;
+  g.gate_s = h->d_gate_s;
+  g.up_s = h->d_up_s;
+  g.down_s = h->d_down_s;
+  g.H = h->H;
+  g.I = h->I;
+  g.hq = h->d_hq;
+  g.hs = h->d_hs;
+  g.hs_stride = h->hs_stride;
+  g.y = h->d_y;
+  g.err = h->d_err;
+  return g;
+}
+
+// Launches gate/up (+SwiGLU+requant) and down for experts [e_begin, e_end) on `s`.
+// `max_tiles` bounds the number of 128-row tiles in the range (host-side, no sync).
+slp_status launch_experts(L* h, cudaStream_t s, int e_begin, int e_end, int T, int max_tiles) {
+  if (h->cfg.gemm_impl == 1) {
+    slp::GemmArgs g0 = gemm_args(h, 0, e_begin, e_end, T), g1 = gemm_args(h, 1, e_begin, e_end, T);
+    dim3 grid0(h->I / 128, max_tiles * 4), grid1(h->H / 128, max_tiles * 4);
+    slp::gemm_simt_kernel<0><<<grid0, 256, 0, s>>>(g0);
+    slp::gemm_simt_kernel<1><<<grid1, 256, 0, s>>>(g1);
+  } else {
+    slp::GemmArgs g0 = gemm_args(h, 0, e_begin, e_end, T), g1 = gemm_args(h, 1, e_begin, e_end, T);
+    const int nt0 = h->I / 128, nt1 = (h->H + 255) / 256;
+    const int grid0 = std::max(1, std::min(h->num_sms, max_tiles * nt0));
+    const int grid1 = std::max(1, std::min(h->num_sms, max_tiles * nt1));
+    slp::tc::gemm_tc_kernel<0><<<grid0, slp::tc::kThreads, slp::tc::kSmemBytes, s>>>(h->tm_xq, h->tm_wgu, g0);
+    slp::tc::gemm_tc_kernel<1><<<grid1, slp::tc::kThreads, slp::tc::kSmemBytes, s>>>(h->tm_hq, h->tm_wd, g1);
+  }
+  CU_TRY(cudaGetLastError());
+  h->stats.gemm_launches += 2;
+  h->stats.kernel_launches += 2;
+  return SLP_OK;
+}
+
+slp_status copy_expert(L* h, int e) {
+  const size_t IH = static_cast<size_t>(h->I) * h->H;
+  uint8_t* slot = h->d_pool + static_cast<size_t>(1 + e % h->n_stage) * h->slot_bytes;
+  CU_TRY(cudaMemcpyAsync(slot, h->gate_q[e], IH, cudaMemcpyHostToDevice, h->copy_stream));
+  CU_TRY(cudaMemcpyAsync(slot + IH, h->up_q[e], IH, cudaMemcpyHostToDevice, h->copy_stream));
+  CU_TRY(cudaMemcpyAsync(slot + 2 * IH, h->down_q[e], IH, cudaMemcpyHostToDevice, h->copy_stream));
+  h->stats.bytes_copied += static_cast<int64_t>(3 * IH);
+  h->stats.experts_copied += 1;
+  return SLP_OK;
+}
+
+slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t s) {
+  const int E = h->E, k = h->k, H = h->H;
+  const bool shared = h->cfg.n_shared != 0;
+  h->stats = slp_moe_stats{};
+  h->stats.struct_size = sizeof(slp_moe_stats);
+  h->stats.tokens = T;
+  h->stats.residency = h->residency;
+  h->stats_copy_valid = false;
+  auto launched = [&](int n) { h->stats.kernel_launches += n; };
+
+  CU_TRY(cudaEventRecord(h->ev_t[0], s));
+  // ---- a1 router ----
+  {
+    dim3 grid((T + 63) / 64, (E + 63) / 64);
+    slp::router_logits_kernel<<<grid, 256, 0, s>>>(static_cast<const uint16_t*>(hidden), h->d_router_w, h->d_logits, T, H, E);
+    const int warps = 8;
+    const int blocks = (T + warps - 1) / warps;
+    const float* bias = h->cfg.scoring == SLP_SCORE_SIGMOID_BIAS ? h->d_bias : nullptr;
+    if (E <= 128)
+      slp::router_topk_kernel<4><<<blocks, warps * 32, 0, s>>>(h->d_logits, bias, h->d_idx, h->d_w, T, E, k, h->cfg.n_group,
+                                                               h->cfg.topk_group, h->cfg.scoring, h->cfg.norm_topk, h->cfg.routed_scale);
+    else if (E <= 256)
+      slp::router_topk_kernel<8><<<blocks, warps * 32, 0, s>>>(h->d_logits, bias, h->d_idx, h->d_w, T, E, k, h->cfg.n_group,
+                                                               h->cfg.topk_group, h->cfg.scoring, h->cfg.norm_topk, h->cfg.routed_scale);
+    else
+      slp::router_topk_kernel<16><<<blocks, warps * 32, 0, s>>>(h->d_logits, bias, h->d_idx, h->d_w, T, E, k, h->cfg.n_group,
+                                                                h->cfg.topk_group, h->cfg.scoring, h->cfg.norm_topk, h->cfg.routed_scale);
+    launched(2);
+  }
+  // ---- a2 histogram / scan / permute ----
+  const int n_chunks = (T + slp::kChunkTokens - 1) / slp::kChunkTokens;
+  {
+    const int wpb = 4;
+    const int blocks = (n_chunks + wpb - 1) / wpb;
+    const size_t sm = static_cast<size_t>(wpb) * E * sizeof(int32_t);
+    CU_TRY(cudaMemsetAsync(h->d_row_token, 0xFF, static_cast<size_t>(h->rows_max) * sizeof(int32_t), s));
+    slp::permute_hist_kernel<<<blocks, wpb * 32, sm, s>>>(h->d_idx, h->d_chunk, T, k, E);
+    slp::permute_scan_kernel<<<1, 512, 0, s>>>(h->d_chunk, h->d_counts, h->d_row_start, h->d_tile_start, h->d_tile_expert, n_chunks, T,
+                                               E, shared ? 1 : 0);
+    slp::permute_place_kernel<<<blocks, wpb * 32, sm, s>>>(h->d_idx, h->d_chunk, h->d_row_start, h->d_pos, h->d_row_token, T, k, E);
+    launched(3);
+  }
+  // ---- a3 hidden quantisation + scatter into expert order ----
+  slp::quant_scatter_kernel<<<T, 256, 0, s>>>(static_cast<const uint16_t*>(hidden), h->d_pos, h->d_xq, h->d_xs, T, H, k, h->xs_stride);
+  launched(1);
+  CU_TRY(cudaGetLastError());
+  CU_TRY(cudaEventRecord(h->ev_t[1], s));
+
+  const int Tpad_tiles = (T + 127) / 128;
+  const int routed_tiles_bound = (T * k) / 128 + E;
+  h->stats.m_tiles = 0;
+
+  bool skip = h->cfg.skip_empty_experts != 0;
+  if (skip) {
+    CU_TRY(cudaMemcpyAsync(h->h_counts, h->d_counts, E * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+    CU_TRY(cudaStreamSynchronize(s));
+  }
+
+  CU_TRY(cudaEventRecord(h->ev_t[2], s));
+  if (h->residency == SLP_RESIDENT) {
+    slp_status st = launch_experts(h, s, 0, shared ? E + 1 : E, T, routed_tiles_bound + (shared ? Tpad_tiles : 0));
+    if (st != SLP_OK) return st;
+  } else {
+    // ---- a4 streaming engine ----
+    if (shared) {  // resident weights: runs while the first expert copies are in flight
+      slp_status st = launch_experts(h, s, E, E + 1, T, Tpad_tiles);
+      if (st != SLP_OK) return st;
+    }
+    const int epl = h->epl;
+    const int n_ring = static_cast<int>(h->ev_ready.size());
+    bool first_copy = true;
+    for (int e0 = 0, grp = 0; e0 < E; e0 += epl, ++grp) {
+      const int e1 = std::min(E, e0 + epl);
+      const int r = grp % n_ring;
+      int need = 0, rows_bound = 0;
+      for (int e = e0; e < e1; ++e) {
+        const bool want = !skip || h->h_counts[e] > 0;
+        need += want ? 1 : 0;
+        if (skip) rows_bound += (h->h_counts[e] + 127) / 128;
+      }
+      if (need == 0) {
+        h->stats.experts_skipped += e1 - e0;
+        continue;
+      }
+      if (h->free_recorded[r]) CU_TRY(cudaStreamWaitEvent(h->copy_stream, h->ev_free[r], 0));  // OFF -> slot reusable
+      if (first_copy) {
+        CU_TRY(cudaEventRecord(h->ev_copy0, h->copy_stream));
+        first_copy = false;
+      }
+      for (int e = e0; e < e1; ++e) {
+        if (skip && h->h_counts[e] == 0) {
+          h->stats.experts_skipped += 1;
+          continue;
+        }
+        slp_status st = copy_expert(h, e);
+        if (st != SLP_OK) return st;
+      }
+      CU_TRY(cudaEventRecord(h->ev_ready[r], h->copy_stream));  // ON
+      CU_TRY(cudaStreamWaitEvent(s, h->ev_ready[r], 0));
+      const int bound = skip ? rows_bound : std::min(routed_tiles_bound, (T * k) / 128 + (e1 - e0));
+      slp_status st = launch_experts(h, s, e0, e1, T, std::max(1, bound));
+      if (st != SLP_OK) return st;
+      CU_TRY(cudaEventRecord(h->ev_free[r], s));  // OFF
+      h->free_recorded[r] = 1;
+    }
+    if (!first_copy) {
+      CU_TRY(cudaEventRecord(h->ev_copy1, h->copy_stream));
+      h->stats_copy_valid = true;
+    }
+  }
+  CU_TRY(cudaEventRecord(h->ev_t[3], s));
+  // ---- a9 combine ----
+  slp::combine_kernel<<<T, 256, 0, s>>>(h->d_y, h->d_pos, h->d_w, static_cast<__nv_bfloat16*>(out), T, H, k, shared ? 1 : 0);
+  launched(1);
+  CU_TRY(cudaGetLastError());
+  CU_TRY(cudaMemcpyAsync(h->h_err, h->d_err, sizeof(int), cudaMemcpyDeviceToHost, s));
+  CU_TRY(cudaEventRecord(h->ev_t[4], s));
+  CU_TRY(cudaEventRecord(h->ev_done, s));
+  h->in_flight = true;
+  h->last_stream = s;
+  h->last_T = T;
+  return SLP_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* slp_last_error(void) { return g_last_error.c_str(); }
+const char* slp_version(void) { return "slpmoe 0.1 (sm_100a)"; }
+
+slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weights* w, slp_moe_layer** out) {
+  if (!cfg || !w || !out) return fail(SLP_ERR_INVALID_ARG, "NULL argument");
+  if (cfg->struct_size != sizeof(slp_moe_cfg)) return fail(SLP_ERR_INVALID_ARG, "cfg.struct_size %u != %zu", cfg->struct_size, sizeof(slp_moe_cfg));
+  *out = nullptr;
+  const int H = cfg->hidden, E = cfg->n_experts, k = cfg->top_k, I = cfg->moe_intermediate, G = cfg->n_group, Gk = cfg->topk_group;
+  if (H <= 0 || I <= 0 || H % 128 || I % 128 || H / 128 > 1024 || I / 128 > 1024)
+    return fail(SLP_ERR_UNSUPPORTED_SHAPE, "hidden (%d) and moe_intermediate (%d) must be positive multiples of 128", H, I);
+  if (E <= 0 || E > slp::kMaxExperts - 1) return fail(SLP_ERR_UNSUPPORTED_SHAPE, "n_experts %d outside 1..%d", E, slp::kMaxExperts - 1);
+  if (G <= 0 || G > 32 || E % G || Gk <= 0 || Gk > G) return fail(SLP_ERR_UNSUPPORTED_SHAPE, "n_group %d / topk_group %d invalid for %d experts", G, Gk, E);
+  if (k <= 0 || k > 32 || k > E || static_cast<long long>(k) > static_cast<long long>(Gk) * (E / G))
+    return fail(SLP_ERR_UNSUPPORTED_SHAPE, "top_k %d invalid (needs 1..32, <= topk_group * E / n_group)", k);
+  if (cfg->n_shared < 0 || cfg->n_shared > 1 || (cfg->n_shared == 1 && cfg->shared_intermediate != I))
+    return fail(SLP_ERR_UNSUPPORTED_SHAPE, "n_shared must be 0 or 1 with shared_intermediate == moe_intermediate");
+  if (cfg->scoring != SLP_SCORE_SIGMOID_BIAS && cfg->scoring != SLP_SCORE_SOFTMAX) return fail(SLP_ERR_INVALID_ARG, "unknown scoring %d", cfg->scoring);
+  if (cfg->max_tokens <= 0) return fail(SLP_ERR_INVALID_ARG, "max_tokens must be positive");
+  if (cfg->gemm_impl != 0 && cfg->gemm_impl != 1) return fail(SLP_ERR_INVALID_ARG, "gemm_impl must be 0 or 1");
+  int n_stage = cfg->staging_slots == 0 ? E : cfg->staging_slots;
+  if (n_stage < 2 && E >= 2) return fail(SLP_ERR_INVALID_ARG, "staging_slots must be 0 or 2..n_experts");
+  n_stage = std::min(n_stage, E);
+  int epl = cfg->experts_per_launch;
+  if (epl == 0) epl = n_stage == E ? std::min(8, E) : std::max(1, std::min(8, n_stage / 2));
+  if (epl < 1 || epl > n_stage || (n_stage != E && (epl > n_stage / 2 || n_stage % epl)))
+    return fail(SLP_ERR_INVALID_ARG, "experts_per_launch %d invalid for %d staging slots (must divide it, <= half)", epl, n_stage);
+  if (!w->router_w || !w->gate_q || !w->gate_s || !w->up_q || !w->up_s || !w->down_q || !w->down_s)
+    return fail(SLP_ERR_INVALID_ARG, "NULL weight pointer");
+  if (cfg->n_shared && (!w->shared_gate_q || !w->shared_gate_s || !w->shared_up_q || !w->shared_up_s || !w->shared_down_q || !w->shared_down_s))
+    return fail(SLP_ERR_INVALID_ARG, "n_shared == 1 but a shared weight pointer is NULL");
+
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    return fail(SLP_ERR_CUDA, "no CUDA device available (this library has no CPU path)");
+  }
+  if (cfg->device < 0 || cfg->device >= ndev) return fail(SLP_ERR_INVALID_ARG, "device %d out of range", cfg->device);
+  CU_TRY(cudaSetDevice(cfg->device));
+  cudaDeviceProp prop{};
+  CU_TRY(cudaGetDeviceProperties(&prop, cfg->device));
+  if (prop.major != 10) return fail(SLP_ERR_CUDA, "device %d is sm_%d%d; this library is built for sm_100a only", cfg->device, prop.major, prop.minor);
+
+  L* h = new (std::nothrow) L();
+  if (!h) return fail(SLP_ERR_OOM, "out of host memory");
+  h->cfg = *cfg;
+  h->hw = *w;
+  h->H = H; h->E = E; h->k = k; h->I = I; h->Tm = cfg->max_tokens;
+  h->kbH = H / 128; h->kbI = I / 128;
+  h->xs_stride = round_up(h->kbH, 4);
+  h->hs_stride = round_up(h->kbI, 4);
+  h->num_sms = prop.multiProcessorCount;
+  h->slot_bytes = static_cast<size_t>(3) * I * H;
+  const int Tpad = round_up(h->Tm, 128);
+  h->rows_max = Tpad + round_up(h->Tm * k + E * 127, 128);
+  h->tiles_max = h->rows_max / 128 + 1;
+  h->n_chunks_max = (h->Tm + slp::kChunkTokens - 1) / slp::kChunkTokens;
+  h->gate_q.assign(w->gate_q, w->gate_q + E);
+  h->up_q.assign(w->up_q, w->up_q + E);
+  h->down_q.assign(w->down_q, w->down_q + E);
+
+  auto bail = [&](slp_status st) {
+    std::string keep = g_last_error;
+    slp_moe_layer_destroy(h);
+    g_last_error = keep;
+    return st;
+  };
+#define TRY_OR_BAIL(expr)                         \
+  do {                                            \
+    slp_status _s = (expr);                       \
+    if (_s != SLP_OK) return bail(_s);            \
+  } while (0)
+#define CU_OR_BAIL(expr)                                                                                        \
+  do {                                                                                                          \
+    cudaError_t _e = (expr);                                                                                    \
+    if (_e != cudaSuccess)                                                                                      \
+      return bail(fail(_e == cudaErrorMemoryAllocation ? SLP_ERR_OOM : SLP_ERR_CUDA, "%s failed: %s", #expr,    \
+                       cudaGetErrorString(_e)));                                                                \
+  } while (0)
+
+  // pin (or check) the streamed weights
+  const size_t IH = static_cast<size_t>(I) * H;
+  for (int e = 0; e < E; ++e) {
+    if (!h->gate_q[e] || !h->up_q[e] || !h->down_q[e] || !w->gate_s[e] || !w->up_s[e] || !w->down_s[e])
+      return bail(fail(SLP_ERR_INVALID_ARG, "NULL weight pointer for expert %d", e));
+    TRY_OR_BAIL(pin_range(h, h->gate_q[e], IH, "gate_q"));
+    TRY_OR_BAIL(pin_range(h, h->up_q[e], IH, "up_q"));
+    TRY_OR_BAIL(pin_range(h, h->down_q[e], IH, "down_q"));
+  }
+
+  CU_OR_BAIL(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
+  CU_OR_BAIL(cudaStreamCreateWithFlags(&h->own_stream, cudaStreamNonBlocking));
+  CU_OR_BAIL(cudaEventCreateWithFlags(&h->ev_done, cudaEventDisableTiming));
+  for (auto& e : h->ev_t) CU_OR_BAIL(cudaEventCreate(&e));
+  CU_OR_BAIL(cudaEventCreate(&h->ev_copy0));
+  CU_OR_BAIL(cudaEventCreate(&h->ev_copy1));
+
+  // resident tensors: router, bias, all block scales (entry E = shared expert)
+  const size_t sc_gu = static_cast<size_t>(h->kbI) * h->kbH, sc_d = static_cast<size_t>(h->kbH) * h->kbI;
+  CU_OR_BAIL(cudaMalloc(&h->d_router_w, static_cast<size_t>(E) * H * sizeof(float)));
+  CU_OR_BAIL(cudaMemcpy(h->d_router_w, w->router_w, static_cast<size_t>(E) * H * sizeof(float), cudaMemcpyHostToDevice));
+  CU_OR_BAIL(cudaMalloc(&h->d_bias, E * sizeof(float)));
+  if (w->router_bias) CU_OR_BAIL(cudaMemcpy(h->d_bias, w->router_bias, E * sizeof(float), cudaMemcpyHostToDevice));
+  else CU_OR_BAIL(cudaMemset(h->d_bias, 0, E * sizeof(float)));
+  CU_OR_BAIL(cudaMalloc(&h->d_gate_s, (E + 1) * sc_gu * sizeof(float)));
+  CU_OR_BAIL(cudaMalloc(&h->d_up_s, (E + 1) * sc_gu * sizeof(float)));
+  CU_OR_BAIL(cudaMalloc(&h->d_down_s, (E + 1) * sc_d * sizeof(float)));
+  for (int e = 0; e < E; ++e) {
+    CU_OR_BAIL(cudaMemcpy(h->d_gate_s + e * sc_gu, w->gate_s[e], sc_gu * sizeof(float), cudaMemcpyHostToDevice));
+    CU_OR_BAIL(cudaMemcpy(h->d_up_s + e * sc_gu, w->up_s[e], sc_gu * sizeof(float), cudaMemcpyHostToDevice));
+    CU_OR_BAIL(cudaMemcpy(h->d_down_s + e * sc_d, w->down_s[e], sc_d * sizeof(float), cudaMemcpyHostToDevice));
+  }
+  if (cfg->n_shared) {
+    CU_OR_BAIL(cudaMemcpy(h->d_gate_s + E * sc_gu, w->shared_gate_s, sc_gu * sizeof(float), cudaMemcpyHostToDevice));
+    CU_OR_BAIL(cudaMemcpy(h->d_up_s + E * sc_gu, w->shared_up_s, sc_gu * sizeof(float), cudaMemcpyHostToDevice));
+    CU_OR_BAIL(cudaMemcpy(h->d_down_s + E * sc_d, w->shared_down_s, sc_d * sizeof(float), cudaMemcpyHostToDevice));
+  }
+
+  // workspace
+  const size_t Tm = h->Tm, rows = h->rows_max;
+  CU_OR_BAIL(cudaMalloc(&h->d_logits, Tm * E * sizeof(float)));
+  CU_OR_BAIL(cudaMalloc(&h->d_idx, Tm * k * sizeof(int32_t)));
+  CU_OR_BAIL(cudaMalloc(&h->d_w, Tm * k * sizeof(float)));
+  CU_OR_BAIL(cudaMalloc(&h->d_counts, E * sizeof(int32_t)));
+  CU_OR_BAIL(cudaMalloc(&h->d_chunk, static_cast<size_t>(h->n_chunks_max) * E * sizeof(int32_t)));
+  CU_OR_BAIL(cudaMalloc(&h->d_row_start, (E + 2) * sizeof(int32_t)));
+  CU_OR_BAIL(cudaMalloc(&h->d_tile_start, (E + 2) * sizeof(int32_t)));
+  CU_OR_BAIL(cudaMalloc(&h->d_tile_expert, static_cast<size_t>(h->tiles_max) * sizeof(int32_t)));
+  CU_OR_BAIL(cudaMalloc(&h->d_pos, Tm * k * sizeof(int32_t)));
+  CU_OR_BAIL(cudaMalloc(&h->d_row_token, rows * sizeof(int32_t)));
+  CU_OR_BAIL(cudaMalloc(&h->d_xq, rows * H));
+  CU_OR_BAIL(cudaMalloc(&h->d_xs, rows * h->xs_stride * sizeof(float)));
+  CU_OR_BAIL(cudaMalloc(&h->d_hq, rows * I));
+  CU_OR_BAIL(cudaMalloc(&h->d_hs, rows * h->hs_stride * sizeof(float)));
+  CU_OR_BAIL(cudaMalloc(&h->d_y, rows * H * sizeof(__nv_bfloat16)));
+  CU_OR_BAIL(cudaMalloc(&h->d_err, sizeof(int)));
+  CU_OR_BAIL(cudaMemset(h->d_err, 0, sizeof(int)));
+  // padding rows are read by the tensor cores (their outputs are discarded): keep them finite
+  CU_OR_BAIL(cudaMemset(h->d_xq, 0, rows * H));
+  CU_OR_BAIL(cudaMemset(h->d_hq, 0, rows * I));
+  CU_OR_BAIL(cudaMallocHost(&h->h_counts, E * sizeof(int32_t)));
+  CU_OR_BAIL(cudaMallocHost(&h->h_err, sizeof(int)));
+  *h->h_err = 0;
+
+  TRY_OR_BAIL(make_tmap_u8(&h->tm_xq, h->d_xq, H, rows));
+  TRY_OR_BAIL(make_tmap_u8(&h->tm_hq, h->d_hq, I, rows));
+  TRY_OR_BAIL(alloc_pool(h, n_stage, epl));
+
+  CU_OR_BAIL(cudaFuncSetAttribute(slp::tc::gemm_tc_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::tc::kSmemBytes));
+  CU_OR_BAIL(cudaFuncSetAttribute(slp::tc::gemm_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::tc::kSmemBytes));
+  CU_OR_BAIL(cudaDeviceSynchronize());
+#undef TRY_OR_BAIL
+#undef CU_OR_BAIL
+  *out = h;
+  return SLP_OK;
+}
+
+slp_status slp_moe_set_residency(slp_moe_layer* h, slp_residency r) {
+  if (!h) return fail(SLP_ERR_INVALID_ARG, "NULL handle");
+  if (r != SLP_STREAMED && r != SLP_RESIDENT) return fail(SLP_ERR_INVALID_ARG, "unknown residency %d", static_cast<int>(r));
+  CU_TRY(cudaSetDevice(h->cfg.device));
+  slp_status st = wait_idle(h);
+  if (st != SLP_OK) return st;
+  CU_TRY(cudaDeviceSynchronize());
+  if (static_cast<int>(r) == h->residency) return SLP_OK;
+  if (r == SLP_RESIDENT) {
+    st = alloc_pool(h, h->E, h->E);
+    if (st != SLP_OK) return st;
+    h->stats = slp_moe_stats{};
+    for (int e = 0; e < h->E; ++e) {
+      st = copy_expert(h, e);
+      if (st != SLP_OK) return st;
+    }
+    CU_TRY(cudaStreamSynchronize(h->copy_stream));
+  } else {
+    int n_stage = h->cfg.staging_slots == 0 ? h->E : std::min(h->cfg.staging_slots, h->E);
+    int epl = h->cfg.experts_per_launch;
+    if (epl == 0) epl = n_stage == h->E ? std::min(8, h->E) : std::max(1, std::min(8, n_stage / 2));
+    st = alloc_pool(h, n_stage, epl);
+    if (st != SLP_OK) return st;
+  }
+  h->residency = r;
+  return SLP_OK;
+}
+
+slp_status slp_moe_prefill(slp_moe_layer* h, const void* hidden_bf16, int32_t T, void* out_bf16, void* cuda_stream) {
+  if (!h) return fail(SLP_ERR_INVALID_ARG, "NULL handle");
+  if (T < 0 || T > h->Tm) return fail(SLP_ERR_INVALID_ARG, "T = %d outside 0..max_tokens (%d)", T, h->Tm);
+  if (T == 0) return SLP_OK;
+  if (!hidden_bf16 || !out_bf16) return fail(SLP_ERR_INVALID_ARG, "NULL hidden/out");
+  if (hidden_bf16 == out_bf16) return fail(SLP_ERR_INVALID_ARG, "out must not alias hidden");
+  CU_TRY(cudaSetDevice(h->cfg.device));
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  if (h->in_flight) {
+    cudaError_t q = cudaEventQuery(h->ev_done);
+    if (q == cudaSuccess) {
+      h->in_flight = false;
+    } else if (q == cudaErrorNotReady) {
+      if (s != h->last_stream) return fail(SLP_ERR_BUSY, "a call is still in flight on another stream");
+    } else {
+      return fail(SLP_ERR_CUDA, "cudaEventQuery failed: %s", cudaGetErrorString(q));
+    }
+  }
+  return prefill_impl(h, hidden_bf16, T, out_bf16, s);
+}
+
+slp_status slp_moe_prefill_host(slp_moe_layer* h, const void* hidden_host, int32_t T, void* out_host) {
+  if (!h) return fail(SLP_ERR_INVALID_ARG, "NULL handle");
+  if (T < 0 || T > h->Tm) return fail(SLP_ERR_INVALID_ARG, "T = %d outside 0..max_tokens (%d)", T, h->Tm);
+  if (T == 0) return SLP_OK;
+  if (!hidden_host || !out_host) return fail(SLP_ERR_INVALID_ARG, "NULL hidden/out");
+  CU_TRY(cudaSetDevice(h->cfg.device));
+  slp_status st = wait_idle(h);
+  if (st != SLP_OK) return st;
+  const size_t bytes = static_cast<size_t>(h->Tm) * h->H * 2;
+  if (!h->d_e2e_in) {
+    CU_TRY(cudaMalloc(&h->d_e2e_in, bytes));
+    CU_TRY(cudaMalloc(&h->d_e2e_out, bytes));
+  }
+  const size_t n = static_cast<size_t>(T) * h->H * 2;
+  CU_TRY(cudaMemcpyAsync(h->d_e2e_in, hidden_host, n, cudaMemcpyHostToDevice, h->own_stream));
+  st = prefill_impl(h, h->d_e2e_in, T, h->d_e2e_out, h->own_stream);
+  if (st != SLP_OK) return st;
+  CU_TRY(cudaMemcpyAsync(out_host, h->d_e2e_out, n, cudaMemcpyDeviceToHost, h->own_stream));
+  CU_TRY(cudaStreamSynchronize(h->own_stream));
+  h->in_flight = false;
+  return check_kernel_error(h);
+}
+
+slp_status slp_moe_layer_destroy(slp_moe_layer* h) {
+  if (!h) return SLP_OK;
+  cudaSetDevice(h->cfg.device);
+  cudaDeviceSynchronize();
+  free_pool(h);
+  void* ptrs[] = {h->d_router_w, h->d_bias, h->d_gate_s, h->d_up_s, h->d_down_s, h->d_logits, h->d_w, h->d_xs, h->d_hs, h->d_idx,
+                  h->d_counts, h->d_chunk, h->d_row_start, h->d_tile_start, h->d_tile_expert, h->d_pos, h->d_row_token, h->d_xq,
+                  h->d_hq, h->d_y, h->d_err, h->d_e2e_in, h->d_e2e_out};
+  for (void* p : ptrs)
+    if (p) cudaFree(p);
+  if (h->h_counts) cudaFreeHost(h->h_counts);
+  if (h->h_err) cudaFreeHost(h->h_err);
+  for (void* p : h->registered) cudaHostUnregister(p);
+  if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
+  if (h->own_stream) cudaStreamDestroy(h->own_stream);
+  if (h->ev_done) cudaEventDestroy(h->ev_done);
+  for (auto e : h->ev_t)
+    if (e) cudaEventDestroy(e);
+  if (h->ev_copy0) cudaEventDestroy(h->ev_copy0);
+  if (h->ev_copy1) cudaEventDestroy(h->ev_copy1);
+  cudaGetLastError();
+  delete h;
+  return SLP_OK;
+}
+
+slp_status slp_moe_debug_routing(slp_moe_layer* h, int32_t* idx, float* w, int32_t* counts) {
+  if (!h) return fail(SLP_ERR_INVALID_ARG, "NULL handle");
+  CU_TRY(cudaSetDevice(h->cfg.device));
+  slp_status st = wait_idle(h);
+  if (st != SLP_OK) return st;
+  const size_t n = static_cast<size_t>(h->last_T) * h->k;
+  if (idx) CU_TRY(cudaMemcpy(idx, h->d_idx, n * sizeof(int32_t), cudaMemcpyDeviceToHost));
+  if (w) CU_TRY(cudaMemcpy(w, h->d_w, n * sizeof(float), cudaMemcpyDeviceToHost));
+  if (counts) CU_TRY(cudaMemcpy(counts, h->d_counts, h->E * sizeof(int32_t), cudaMemcpyDeviceToHost));
+  return check_kernel_error(h);
+}
+
+slp_status slp_moe_debug_quant_hidden(slp_moe_layer* h, uint8_t* xq, float* xs) {
+  if (!h) return fail(SLP_ERR_INVALID_ARG, "NULL handle");
+  CU_TRY(cudaSetDevice(h->cfg.device));
+  slp_status st = wait_idle(h);
+  if (st != SLP_OK) return st;
+  const int T = h->last_T;
+  if (xq) CU_TRY(cudaMemcpy(xq, h->d_xq, static_cast<size_t>(T) * h->H, cudaMemcpyDeviceToHost));
+  if (xs)
+    CU_TRY(cudaMemcpy2D(xs, h->kbH * sizeof(float), h->d_xs, h->xs_stride * sizeof(float), h->kbH * sizeof(float), T, cudaMemcpyDeviceToHost));
+  return check_kernel_error(h);
+}
+
+slp_status slp_moe_debug_buffer(slp_moe_layer* h, int32_t which, void* dst, size_t bytes, size_t* written) {
+  if (!h || !dst) return fail(SLP_ERR_INVALID_ARG, "NULL argument");
+  CU_TRY(cudaSetDevice(h->cfg.device));
+  slp_status st = wait_idle(h);
+  if (st != SLP_OK) return st;
+  int32_t rs[2] = {0, 0};  // row_start[E+1] = rows in use
+  CU_TRY(cudaMemcpy(rs, h->d_row_start + h->E + 1, sizeof(int32_t), cudaMemcpyDeviceToHost));
+  const size_t rows = static_cast<size_t>(rs[0]), T = h->last_T;
+  const void* src = nullptr;
+  size_t size = 0;
+  switch (which) {
+    case SLP_BUF_COUNTS: src = h->d_counts; size = h->E * sizeof(int32_t); break;
+    case SLP_BUF_ROW_START: src = h->d_row_start; size = (h->E + 1) * sizeof(int32_t); break;
+    case SLP_BUF_POS: src = h->d_pos; size = T * h->k * sizeof(int32_t); break;
+    case SLP_BUF_ROW_TOKEN: src = h->d_row_token; size = rows * sizeof(int32_t); break;
+    case SLP_BUF_HQ: src = h->d_hq; size = rows * h->I; break;
+    case SLP_BUF_HS: src = h->d_hs; size = rows * h->hs_stride * sizeof(float); break;
+    case SLP_BUF_Y: src = h->d_y; size = rows * h->H * 2; break;
+    case SLP_BUF_LOGITS: src = h->d_logits; size = T * h->E * sizeof(float); break;
+    default: return fail(SLP_ERR_INVALID_ARG, "unknown buffer id %d", which);
+  }
+  const size_t n = std::min(size, bytes);
+  if (n) CU_TRY(cudaMemcpy(dst, src, n, cudaMemcpyDeviceToHost));
+  if (written) *written = size;
+  return check_kernel_error(h);
+}
+
+slp_status slp_moe_get_stats(slp_moe_layer* h, slp_moe_stats* stats) {
+  if (!h || !stats) return fail(SLP_ERR_INVALID_ARG, "NULL argument");
+  if (stats->struct_size != sizeof(slp_moe_stats)) return fail(SLP_ERR_INVALID_ARG, "stats.struct_size mismatch");
+  CU_TRY(cudaSetDevice(h->cfg.device));
+  slp_status st = wait_idle(h);
+  if (st != SLP_OK) return st;
+  if (h->last_T > 0) {
+    CU_TRY(cudaEventSynchronize(h->ev_t[4]));
+    CU_TRY(cudaEventElapsedTime(&h->stats.ms_total, h->ev_t[0], h->ev_t[4]));
+    CU_TRY(cudaEventElapsedTime(&h->stats.ms_route, h->ev_t[0], h->ev_t[1]));
+    CU_TRY(cudaEventElapsedTime(&h->stats.ms_experts, h->ev_t[2], h->ev_t[3]));
+    CU_TRY(cudaEventElapsedTime(&h->stats.ms_combine, h->ev_t[3], h->ev_t[4]));
+    if (h->stats_copy_valid) {
+      CU_TRY(cudaEventSynchronize(h->ev_copy1));
+      CU_TRY(cudaEventElapsedTime(&h->stats.ms_copy_span, h->ev_copy0, h->ev_copy1));
+    }
+    int32_t ts[1] = {0};
+    CU_TRY(cudaMemcpy(ts, h->d_tile_start + h->E + 1, sizeof(int32_t), cudaMemcpyDeviceToHost));
+    h->stats.m_tiles = ts[0];
+  }
+  *stats = h->stats;
+  stats->struct_size = sizeof(slp_moe_stats);
+  return check_kernel_error(h);
+}
+
+slp_status slp_measure_h2d(int32_t device, size_t chunk_bytes, size_t total_bytes, int32_t repeats, double* gbs) {
+  if (!gbs || chunk_bytes == 0 || total_bytes < chunk_bytes || repeats <= 0) return fail(SLP_ERR_INVALID_ARG, "bad arguments");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
+    cudaGetLastError();
+    return fail(SLP_ERR_CUDA, "no such CUDA device %d", device);
+  }
+  CU_TRY(cudaSetDevice(device));
+  const size_t n_chunks = total_bytes / chunk_bytes;
+  void *hbuf = nullptr, *dbuf = nullptr;
+  cudaStream_t s = nullptr;
+  cudaEvent_t a = nullptr, b = nullptr;
+  CU_TRY(cudaMallocHost(&hbuf, n_chunks * chunk_bytes));
+  memset(hbuf, 1, n_chunks * chunk_bytes);
+  slp_status st = SLP_OK;
+  double best = 0;
+  if (cudaMalloc(&dbuf, n_chunks * chunk_bytes) != cudaSuccess || cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking) != cudaSuccess ||
+      cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) {
+    st = fail(SLP_ERR_CUDA, "setup failed: %s", cudaGetErrorString(cudaGetLastError()));
+  } else {
+    for (int r = 0; r < repeats + 1 && st == SLP_OK; ++r) {
+      cudaEventRecord(a, s);
+      for (size_t c = 0; c < n_chunks; ++c)
+        cudaMemcpyAsync(static_cast<char*>(dbuf) + c * chunk_bytes, static_cast<char*>(hbuf) + c * chunk_bytes, chunk_bytes,
+                        cudaMemcpyHostToDevice, s);
+      cudaEventRecord(b, s);
+      if (cudaEventSynchronize(b) != cudaSuccess) {
+        st = fail(SLP_ERR_CUDA, "copy failed: %s", cudaGetErrorString(cudaGetLastError()));
+        break;
+      }
+      float ms = 0;
+      cudaEventElapsedTime(&ms, a, b);
+      if (r > 0) best = std::max(best, static_cast<double>(n_chunks * chunk_bytes) / (ms * 1e-3) / 1e9);
+    }
+  }
+  if (a) cudaEventDestroy(a);
+  if (b) cudaEventDestroy(b);
+  if (s) cudaStreamDestroy(s);
+  if (dbuf) cudaFree(dbuf);
+  cudaFreeHost(hbuf);
+  *gbs = best;
+  return st;
+}
+
+}  // extern "C"

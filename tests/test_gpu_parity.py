@@ -1,0 +1,201 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the CPU oracle, element by element,
+on the same seeded inputs, with the north_star acceptance rule (oracle/acceptance.py).
+
+Sizes: config 0 (tiny), a reduced DeepSeek-V3-like layer that spans several 128-row tiles with a
+ragged tail and a shared expert, a reduced softmax layer (config 4's routing), and the skewed
+config-3 recipe at reduced size (empty experts, 1-3-row experts).  Full-size sampled checks are in
+test_gpu_fullsize.py.
+"""
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import moe_layer, permutation
+from oracle.acceptance import compare_routing, compare_output
+from paper_2606_10493_b200 import SlpMoeLayer, SlpError, inputs
+
+pytestmark = pytest.mark.gpu
+
+
+def small_dsv3(**kw):
+    base = dict(name="mini_dsv3", T=300, H=512, E=32, k=4, G=4, Gk=2, I=256, n_shared=1,
+                scoring="sigmoid_bias", norm_topk=True, routed_scale=2.5, seed=11, bias="normal",
+                mode="streamed")
+    base.update(kw)
+    return inputs.LayerConfig(**base)
+
+
+CASES = {
+    "cfg0": inputs.CONFIGS[0],
+    "mini_dsv3": small_dsv3(),
+    "mini_dsv3_ragged": small_dsv3(T=1000, seed=12, H=768, I=384),
+    "mini_softmax": small_dsv3(name="mini_softmax", T=513, H=256, E=16, k=4, G=1, Gk=1, I=128, n_shared=0,
+                               scoring="softmax", routed_scale=1.0, bias="none", seed=13),
+    "mini_zipf": small_dsv3(name="mini_zipf", T=2048, H=256, E=64, k=8, G=8, Gk=4, I=128, bias="zipf", seed=14),
+}
+
+_cache = {}
+
+
+def problem(name):
+    if name not in _cache:
+        cfg = CASES[name]
+        W = inputs.make_weights(cfg, device="cpu", pin=True)
+        hidden = inputs.make_hidden(cfg, device="cpu")
+        ref = moe_layer(inputs.hidden_as_bits(hidden), inputs.weights_as_numpy(W), top_k=cfg.k,
+                        n_group=cfg.G, topk_group=cfg.Gk, scoring=cfg.scoring,
+                        norm_topk=cfg.norm_topk, routed_scale=cfg.routed_scale)
+        _cache[name] = (cfg, W, hidden, ref)
+    return _cache[name]
+
+
+def run_gpu(cfg, W, hidden, mode, **kw):
+    layer = SlpMoeLayer(cfg, W, device=0, **kw)
+    try:
+        layer.set_residency(mode)
+        out = layer.prefill(hidden.cuda())
+        torch.cuda.synchronize()
+        idx, w, counts = layer.debug_routing(hidden.shape[0])
+        xq, xs = layer.debug_quant_hidden(hidden.shape[0])
+        extra = dict(pos=layer.debug_buffer("pos", np.int32).reshape(hidden.shape[0], cfg.k),
+                     row_start=layer.debug_buffer("row_start", np.int32),
+                     row_token=layer.debug_buffer("row_token", np.int32),
+                     stats=layer.stats())
+    finally:
+        layer.close()
+    return inputs.hidden_as_bits(out), idx, w, counts, xq, xs, extra
+
+
+def check(name, mode, **kw):
+    cfg, W, hidden, ref = problem(name)
+    out, idx, w, counts, xq, xs, extra = run_gpu(cfg, W, hidden, mode, **kw)
+    r = compare_routing(idx, w, ref["route"])
+    o = compare_output(out, ref["out_f64"], r["members_equal"])
+    print(name, mode, kw, {k: v for k, v in r.items() if k != "members_equal"}, o, extra["stats"])
+    assert r["passed"], r
+    assert o["passed"], o
+    return r, o
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_substeps_bit_exact(name):
+    """Router indices (outside near-ties), quantised hidden bytes + scales (bit-exact, Q12) and
+    the permutation (true inverse, expert-contiguous, ascending token id, 128-aligned ranges)."""
+    cfg, W, hidden, ref = problem(name)
+    out, idx, w, counts, xq, xs, extra = run_gpu(cfg, W, hidden, "resident", gemm_impl=1)
+    r = compare_routing(idx, w, ref["route"])
+    assert r["passed"], r
+    assert np.array_equal(xq, ref["xq"])
+    assert np.array_equal(xs, ref["xs"])
+    T, k, E = cfg.T, cfg.k, cfg.E
+    pos, row_start, row_token = extra["pos"], extra["row_start"], extra["row_token"]
+    assert counts.sum() == T * k
+    assert np.array_equal(counts, np.bincount(idx.reshape(-1), minlength=E))
+    assert (row_start[:E] % 128 == 0).all() and row_start[E] == 0
+    assert np.array_equal(row_token[pos], np.repeat(np.arange(T)[:, None], k, axis=1))      # true inverse
+    assert len(np.unique(pos)) == T * k
+    _, offsets, perm, pos_ref = permutation(idx, E)                                            # O8 on the GPU's idx
+    for e in range(E):
+        rows = row_token[row_start[e]:row_start[e] + counts[e]]
+        assert np.array_equal(rows, perm[offsets[e]:offsets[e + 1]])                           # ascending token id
+        pad = row_token[row_start[e] + counts[e]:row_start[e] + (counts[e] + 127) // 128 * 128]
+        assert (pad == -1).all()
+    ee = idx
+    assert np.array_equal(pos - row_start[ee], pos_ref - offsets[ee])
+
+
+@pytest.mark.parametrize("name", list(CASES))
+@pytest.mark.parametrize("mode", ["resident", "streamed"])
+def test_layer_parity_simt(name, mode):
+    check(name, mode, gemm_impl=1)
+
+
+@pytest.mark.parametrize("name", list(CASES))
+@pytest.mark.parametrize("mode", ["resident", "streamed"])
+def test_layer_parity_tcgen05(name, mode):
+    check(name, mode, gemm_impl=0)
+
+
+@pytest.mark.parametrize("kw", [dict(staging_slots=2, experts_per_launch=1),
+                                dict(staging_slots=8, experts_per_launch=4),
+                                dict(staging_slots=4, experts_per_launch=2, skip_empty_experts=True),
+                                dict(skip_empty_experts=True)])
+def test_streaming_ring_variants(kw):
+    """Ring length 2 (the paper's ping-pong), partial rings, empty-expert skipping."""
+    check("mini_zipf", "streamed", **kw)
+    check("mini_dsv3_ragged", "streamed", **kw)
+
+
+def test_run_to_run_bitwise_and_chunking():
+    """Bitwise determinism, and Q20: chunked prefill == single pass, bit for bit."""
+    cfg, W, hidden, ref = problem("mini_dsv3_ragged")
+    layer = SlpMoeLayer(cfg, W, device=0)
+    try:
+        x = hidden.cuda()
+        for mode in ("resident", "streamed"):
+            layer.set_residency(mode)
+            a = layer.prefill(x).clone()
+            b = layer.prefill(x).clone()
+            torch.cuda.synchronize()
+            assert torch.equal(a.view(torch.int16), b.view(torch.int16))
+            parts = []
+            for r0 in range(0, cfg.T, 256):
+                parts.append(layer.prefill(x[r0:r0 + 256].contiguous()).clone())
+            torch.cuda.synchronize()
+            assert torch.equal(torch.cat(parts).view(torch.int16), a.view(torch.int16))
+    finally:
+        layer.close()
+
+
+def test_poisoned_unused_experts():
+    """NaN bytes in the weights of experts that receive no token must not reach the output."""
+    cfg, W, hidden, ref = problem("mini_zipf")
+    unused = np.nonzero(ref["route"]["counts"] == 0)[0]
+    assert len(unused) > 0
+    Wp = {k: (v.clone().pin_memory() if isinstance(v, torch.Tensor) else v) for k, v in W.items()}
+    for e in unused:
+        for key in ("gate_q", "up_q", "down_q"):
+            Wp[key][e].fill_(0x7F)
+    for mode in ("resident", "streamed"):
+        out, idx, w, *_ = run_gpu(cfg, Wp, hidden, mode)
+        r = compare_routing(idx, w, ref["route"])
+        o = compare_output(out, ref["out_f64"], r["members_equal"])
+        assert o["finite"] and o["passed"], o
+
+
+def test_host_entry_point_and_stats():
+    cfg, W, hidden, ref = problem("mini_dsv3")
+    layer = SlpMoeLayer(cfg, W, device=0)
+    try:
+        hin = hidden.pin_memory()
+        hout = torch.empty_like(hin).pin_memory()
+        layer.prefill_host(hin, hout)
+        st = layer.stats()
+        idx, w, _ = layer.debug_routing(cfg.T)
+    finally:
+        layer.close()
+    r = compare_routing(idx, w, ref["route"])
+    o = compare_output(inputs.hidden_as_bits(hout), ref["out_f64"], r["members_equal"])
+    assert o["passed"], o
+    assert st["experts_copied"] == cfg.E and st["bytes_copied"] == cfg.E * 3 * cfg.I * cfg.H
+    assert st["gemm_launches"] > 0 and st["kernel_launches"] > st["gemm_launches"]
+
+
+def test_error_paths():
+    cfg, W, hidden, _ = problem("cfg0")
+    bad = inputs.LayerConfig(**{**cfg.__dict__, "H": 200})
+    with pytest.raises(SlpError) as ei:
+        SlpMoeLayer(bad, W, device=0)
+    assert ei.value.status == -2
+    layer = SlpMoeLayer(cfg, W, device=0)
+    try:
+        x = hidden.cuda()
+        with pytest.raises(SlpError):
+            layer.prefill(torch.cat([x, x]))                      # T > max_tokens
+        out = torch.full_like(x, 7.0)
+        layer.prefill(x[:0], out[:0])                              # T == 0 touches nothing
+        torch.cuda.synchronize()
+        assert (out == 7.0).all()
+    finally:
+        layer.close()
