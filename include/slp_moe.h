@@ -120,6 +120,9 @@ typedef struct {
   int32_t gemm_launches;      /* grouped-GEMM kernel launches in the call */
   int32_t kernel_launches;    /* all kernel launches in the call */
   int32_t m_tiles;            /* 128-row tiles over all experts incl. shared */
+  int32_t timed_gemm_pairs;   /* gate/up + down launch pairs bracketed by CUDA events on the caller's stream */
+  float ms_gateup_sum;        /* sum over those launches of the gate/up (+SwiGLU+requant) kernel time */
+  float ms_down_sum;          /* same for the down kernel */
 } slp_moe_stats;
 
 /* Buffers readable through slp_moe_debug_buffer (parity / evidence; layouts in DESIGN.md §5). */
@@ -130,7 +133,7 @@ typedef enum {
   SLP_BUF_ROW_TOKEN = 3,   /* int32 [rows] token id of each workspace row (-1 = padding) */
   SLP_BUF_HQ = 4,          /* uint8 [rows, I] requantised SwiGLU output */
   SLP_BUF_HS = 5,          /* float [rows, ceil4(I/128)] its scales */
-  SLP_BUF_Y = 6,           /* bf16  [rows, H] per-row expert outputs */
+  SLP_BUF_Y = 6,           /* float [rows, H] per-row expert outputs */
   SLP_BUF_LOGITS = 7       /* float [T, E] router logits */
 } slp_debug_buffer_id;
 

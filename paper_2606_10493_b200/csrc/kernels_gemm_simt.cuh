@@ -33,7 +33,7 @@ struct GemmArgs {
   uint8_t* hq;                 // [rows, I]
   float* hs;                   // [rows, hs_stride]
   int hs_stride;
-  __nv_bfloat16* y;            // [rows, H]
+  float* y;                    // [rows, H] fp32
   int* err;
 };
 
@@ -47,7 +47,7 @@ __device__ __forceinline__ float e4m3_to_float(uint8_t c) {
 
 __device__ __forceinline__ float silu_mul(float g, float u) { return g / (1.0f + expf(-g)) * u; }
 
-// kMode 0: gate/up + SwiGLU + requant -> hq, hs.  kMode 1: down -> y (bf16).
+// kMode 0: gate/up + SwiGLU + requant -> hq, hs.  kMode 1: down -> y (fp32).
 // Block: 32 rows x 128 output channels, 256 threads; thread (ty, tx) owns rows ty*4..+3 and
 // channels tx, tx+32, tx+64, tx+96, so one warp covers all 128 channels of its 4 rows.
 template <int kMode>
@@ -145,7 +145,7 @@ __global__ void __launch_bounds__(256) gemm_simt_kernel(GemmArgs g) {
       }
     } else if (r < nrows) {
 #pragma unroll
-      for (int j = 0; j < 4; ++j) g.y[row * g.H + nb * BC + tx + 32 * j] = __float2bfloat16_rn(acc0[i][j]);
+      for (int j = 0; j < 4; ++j) g.y[row * g.H + nb * BC + tx + 32 * j] = acc0[i][j];
     }
   }
 }

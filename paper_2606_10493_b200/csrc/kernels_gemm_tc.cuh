@@ -17,7 +17,8 @@
 // kMode 0 (gate/up): B = [gate rows n0..n0+127 | up rows n0..n0+127] of the expert; epilogue
 //   h = silu(g) * u, row amax over the 128 channels, s = amax / 448, e4m3(h / s) -> hq, hs
 //   ("SiLU(.) (.)"; fused requantisation, Q14).
-// kMode 1 (down):   B = down rows n0..n0+255; epilogue bf16 store of Y.
+// kMode 1 (down):   B = down rows n0..n0+255; epilogue fp32 store of Y (kept in fp32 so that the
+//   only bf16 rounding of the layer is the final one in the combine).
 #pragma once
 #include <cstdint>
 #include <cuda.h>
@@ -242,17 +243,9 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
       } else {
         const int c0 = nt * BN + half * 128;
         if (row_ok && c0 < g.H) {
-          uint4* dst = reinterpret_cast<uint4*>(g.y + row * g.H + c0);
+          float4* dst = reinterpret_cast<float4*>(g.y + row * g.H + c0);
 #pragma unroll
-          for (int i = 0; i < 16; ++i) {
-            uint32_t o[4];
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              __nv_bfloat162 p = __floats2bfloat162_rn(acc[8 * i + 2 * j], acc[8 * i + 2 * j + 1]);
-              o[j] = *reinterpret_cast<uint32_t*>(&p);
-            }
-            dst[i] = make_uint4(o[0], o[1], o[2], o[3]);
-          }
+          for (int i = 0; i < 32; ++i) dst[i] = make_float4(acc[4 * i], acc[4 * i + 1], acc[4 * i + 2], acc[4 * i + 3]);
         }
       }
     }

@@ -353,10 +353,10 @@ __global__ void __launch_bounds__(256) quant_scatter_kernel(const uint16_t* __re
 
 // ---------------------------------------------------------------------------------------------
 // a9: weighted combine.  out[t] = sum_j w[t,j] * Y[pos[t,j]] (fixed j order, fp32 FMA) + Y[t]
-// (shared expert row, weight 1), rounded once to bf16.  Gather-based, no atomics.
+// (shared expert row, weight 1); Y is fp32 and the sum is rounded once to bf16.  Gather-based, no atomics.
 // (PAPER.md:92 step 5 "A final weighted sum"; "router-weighted accumulation in F32".)
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) combine_kernel(const __nv_bfloat16* __restrict__ y, const int32_t* __restrict__ pos,
+__global__ void __launch_bounds__(256) combine_kernel(const float* __restrict__ y, const int32_t* __restrict__ pos,
                                                       const float* __restrict__ w, __nv_bfloat16* __restrict__ out, int T, int H,
                                                       int k, int has_shared) {
   const int t = blockIdx.x;
@@ -367,34 +367,21 @@ __global__ void __launch_bounds__(256) combine_kernel(const __nv_bfloat16* __res
     s_w[threadIdx.x] = w[static_cast<size_t>(t) * k + threadIdx.x];
   }
   __syncthreads();
-  for (int c = threadIdx.x * 8; c < H; c += blockDim.x * 8) {
-    float acc[8] = {};
+  for (int c = threadIdx.x * 4; c < H; c += blockDim.x * 4) {
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
     for (int j = 0; j < k; ++j) {
-      const uint4 raw = *reinterpret_cast<const uint4*>(y + static_cast<size_t>(s_row[j]) * H + c);
-      const uint32_t r[4] = {raw.x, raw.y, raw.z, raw.w};
+      const float4 v = *reinterpret_cast<const float4*>(y + static_cast<size_t>(s_row[j]) * H + c);
       const float wj = s_w[j];
-#pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        acc[2 * i] = fmaf(wj, __uint_as_float(r[i] << 16), acc[2 * i]);
-        acc[2 * i + 1] = fmaf(wj, __uint_as_float(r[i] & 0xFFFF0000u), acc[2 * i + 1]);
-      }
+      acc.x = fmaf(wj, v.x, acc.x); acc.y = fmaf(wj, v.y, acc.y);
+      acc.z = fmaf(wj, v.z, acc.z); acc.w = fmaf(wj, v.w, acc.w);
     }
     if (has_shared) {
-      const uint4 raw = *reinterpret_cast<const uint4*>(y + static_cast<size_t>(t) * H + c);
-      const uint32_t r[4] = {raw.x, raw.y, raw.z, raw.w};
-#pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        acc[2 * i] += __uint_as_float(r[i] << 16);
-        acc[2 * i + 1] += __uint_as_float(r[i] & 0xFFFF0000u);
-      }
+      const float4 v = *reinterpret_cast<const float4*>(y + static_cast<size_t>(t) * H + c);
+      acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
     }
-    uint32_t o[4];
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      __nv_bfloat162 p = __floats2bfloat162_rn(acc[2 * i], acc[2 * i + 1]);
-      o[i] = *reinterpret_cast<uint32_t*>(&p);
-    }
-    *reinterpret_cast<uint4*>(out + static_cast<size_t>(t) * H + c) = make_uint4(o[0], o[1], o[2], o[3]);
+    __nv_bfloat162 lo = __floats2bfloat162_rn(acc.x, acc.y), hi = __floats2bfloat162_rn(acc.z, acc.w);
+    *reinterpret_cast<uint2*>(out + static_cast<size_t>(t) * H + c) =
+        make_uint2(*reinterpret_cast<uint32_t*>(&lo), *reinterpret_cast<uint32_t*>(&hi));
   }
 }
 

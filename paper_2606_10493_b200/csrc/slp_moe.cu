@@ -102,7 +102,7 @@ struct slp_moe_layer {
   int32_t *d_idx = nullptr, *d_counts = nullptr, *d_chunk = nullptr, *d_row_start = nullptr, *d_tile_start = nullptr,
           *d_tile_expert = nullptr, *d_pos = nullptr, *d_row_token = nullptr;
   uint8_t *d_xq = nullptr, *d_hq = nullptr;
-  __nv_bfloat16* d_y = nullptr;
+  float* d_y = nullptr;
   int* d_err = nullptr;
   void *d_e2e_in = nullptr, *d_e2e_out = nullptr;
   int32_t* h_counts = nullptr;  // pinned
@@ -119,6 +119,8 @@ struct slp_moe_layer {
   int last_T = 0;
   slp_moe_stats stats{};
   bool stats_copy_valid = false;
+  std::vector<cudaEvent_t> ev_k;  // 3 events per expert launch pair: before gate/up, between, after down
+  int ev_k_used = 0;
 };
 
 namespace {
@@ -241,8 +243,15 @@ slp_status launch_experts(L* h, cudaStream_t s, int e_begin, int e_end, int T, i
     const int nt0 = h->I / 128, nt1 = (h->H + 255) / 256;
     const int grid0 = std::max(1, std::min(h->num_sms, max_tiles * nt0));
     const int grid1 = std::max(1, std::min(h->num_sms, max_tiles * nt1));
+    cudaEvent_t* ev = (h->ev_k_used + 3 <= static_cast<int>(h->ev_k.size())) ? &h->ev_k[h->ev_k_used] : nullptr;
+    if (ev) cudaEventRecord(ev[0], s);
     slp::tc::gemm_tc_kernel<0><<<grid0, slp::tc::kThreads, slp::tc::kSmemBytes, s>>>(h->tm_xq, h->tm_wgu, g0);
+    if (ev) cudaEventRecord(ev[1], s);
     slp::tc::gemm_tc_kernel<1><<<grid1, slp::tc::kThreads, slp::tc::kSmemBytes, s>>>(h->tm_hq, h->tm_wd, g1);
+    if (ev) {
+      cudaEventRecord(ev[2], s);
+      h->ev_k_used += 3;
+    }
   }
   CU_TRY(cudaGetLastError());
   h->stats.gemm_launches += 2;
@@ -269,6 +278,7 @@ slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t
   h->stats.tokens = T;
   h->stats.residency = h->residency;
   h->stats_copy_valid = false;
+  h->ev_k_used = 0;
   auto launched = [&](int n) { h->stats.kernel_launches += n; };
 
   CU_TRY(cudaEventRecord(h->ev_t[0], s));
@@ -484,6 +494,8 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
   for (auto& e : h->ev_t) CU_OR_BAIL(cudaEventCreate(&e));
   CU_OR_BAIL(cudaEventCreate(&h->ev_copy0));
   CU_OR_BAIL(cudaEventCreate(&h->ev_copy1));
+  h->ev_k.resize(3 * (E + 2));
+  for (auto& e : h->ev_k) CU_OR_BAIL(cudaEventCreate(&e));
 
   // resident tensors: router, bias, all block scales (entry E = shared expert)
   const size_t sc_gu = static_cast<size_t>(h->kbI) * h->kbH, sc_d = static_cast<size_t>(h->kbH) * h->kbI;
@@ -522,7 +534,7 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
   CU_OR_BAIL(cudaMalloc(&h->d_xs, rows * h->xs_stride * sizeof(float)));
   CU_OR_BAIL(cudaMalloc(&h->d_hq, rows * I));
   CU_OR_BAIL(cudaMalloc(&h->d_hs, rows * h->hs_stride * sizeof(float)));
-  CU_OR_BAIL(cudaMalloc(&h->d_y, rows * H * sizeof(__nv_bfloat16)));
+  CU_OR_BAIL(cudaMalloc(&h->d_y, rows * H * sizeof(float)));
   CU_OR_BAIL(cudaMalloc(&h->d_err, sizeof(int)));
   CU_OR_BAIL(cudaMemset(h->d_err, 0, sizeof(int)));
   // padding rows are read by the tensor cores (their outputs are discarded): keep them finite
@@ -637,6 +649,8 @@ slp_status slp_moe_layer_destroy(slp_moe_layer* h) {
     if (e) cudaEventDestroy(e);
   if (h->ev_copy0) cudaEventDestroy(h->ev_copy0);
   if (h->ev_copy1) cudaEventDestroy(h->ev_copy1);
+  for (auto e : h->ev_k)
+    if (e) cudaEventDestroy(e);
   cudaGetLastError();
   delete h;
   return SLP_OK;
@@ -683,7 +697,7 @@ slp_status slp_moe_debug_buffer(slp_moe_layer* h, int32_t which, void* dst, size
     case SLP_BUF_ROW_TOKEN: src = h->d_row_token; size = rows * sizeof(int32_t); break;
     case SLP_BUF_HQ: src = h->d_hq; size = rows * h->I; break;
     case SLP_BUF_HS: src = h->d_hs; size = rows * h->hs_stride * sizeof(float); break;
-    case SLP_BUF_Y: src = h->d_y; size = rows * h->H * 2; break;
+    case SLP_BUF_Y: src = h->d_y; size = rows * h->H * sizeof(float); break;
     case SLP_BUF_LOGITS: src = h->d_logits; size = T * h->E * sizeof(float); break;
     default: return fail(SLP_ERR_INVALID_ARG, "unknown buffer id %d", which);
   }
@@ -708,6 +722,15 @@ slp_status slp_moe_get_stats(slp_moe_layer* h, slp_moe_stats* stats) {
     if (h->stats_copy_valid) {
       CU_TRY(cudaEventSynchronize(h->ev_copy1));
       CU_TRY(cudaEventElapsedTime(&h->stats.ms_copy_span, h->ev_copy0, h->ev_copy1));
+    }
+    h->stats.ms_gateup_sum = h->stats.ms_down_sum = 0.f;
+    h->stats.timed_gemm_pairs = h->ev_k_used / 3;
+    for (int i = 0; i + 3 <= h->ev_k_used; i += 3) {
+      float a = 0.f, b = 0.f;
+      CU_TRY(cudaEventElapsedTime(&a, h->ev_k[i], h->ev_k[i + 1]));
+      CU_TRY(cudaEventElapsedTime(&b, h->ev_k[i + 1], h->ev_k[i + 2]));
+      h->stats.ms_gateup_sum += a;
+      h->stats.ms_down_sum += b;
     }
     int32_t ts[1] = {0};
     CU_TRY(cudaMemcpy(ts, h->d_tile_start + h->E + 1, sizeof(int32_t), cudaMemcpyDeviceToHost));

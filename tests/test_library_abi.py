@@ -34,7 +34,7 @@ def test_struct_sizes_match_header(built):
     # 19 four-byte fields / 14 pointers / see header
     assert ctypes.sizeof(binding._Cfg) == 19 * 4
     assert ctypes.sizeof(binding._HostWeights) == 14 * 8
-    assert ctypes.sizeof(binding.Stats) == 64
+    assert ctypes.sizeof(binding.Stats) == 80
 
 
 def test_invalid_arguments_are_reported(built):
