@@ -135,6 +135,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-resident-extra", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
     ap.add_argument("--gemm-impl", type=int, default=0)
     ap.add_argument("--staging-slots", type=int, default=0)
     ap.add_argument("--experts-per-launch", type=int, default=0)
@@ -274,23 +275,25 @@ def main():
                                   "frac": step_gbs / h2d_peak, "peak_source": "slp_measure_h2d, pinned, per-matrix chunks, best of 5"}
 
     # end-to-end through the host entry point: hidden from pinned host memory, result read back
-    hin = hidden.cpu().pin_memory()
-    hout = torch.empty_like(hin).pin_memory()
-    for _ in range(max(1, args.warmup // 2)):
-        layer.prefill_host(hin, hout)
-    barrier()
-    t0 = time.perf_counter()
-    n_e2e = max(2, args.steps // 2)
-    for _ in range(n_e2e):
-        layer.prefill_host(hin, hout)
-    e2e_s = (time.perf_counter() - t0) / n_e2e
-    if world > 1:
-        t = torch.tensor([e2e_s], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
-    e2e = {"value": world * cfg.T / e2e_s, "unit": "tokens/s",
-           "h2d_bytes_per_step": cfg.T * cfg.H * 2 + (st["bytes_copied"] if mode == "streamed" else 0),
-           "d2h_bytes_per_step": cfg.T * cfg.H * 2}
+    e2e = None
+    if not args.no_e2e:
+        hin = hidden.cpu().pin_memory()
+        hout = torch.empty_like(hin).pin_memory()
+        for _ in range(max(1, args.warmup // 2)):
+            layer.prefill_host(hin, hout)
+        barrier()
+        t0 = time.perf_counter()
+        n_e2e = max(2, args.steps // 2)
+        for _ in range(n_e2e):
+            layer.prefill_host(hin, hout)
+        e2e_s = (time.perf_counter() - t0) / n_e2e
+        if world > 1:
+            t = torch.tensor([e2e_s], device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e2e_s = float(t.item())
+        e2e = {"value": world * cfg.T / e2e_s, "unit": "tokens/s",
+               "h2d_bytes_per_step": cfg.T * cfg.H * 2 + (st["bytes_copied"] if mode == "streamed" else 0),
+               "d2h_bytes_per_step": cfg.T * cfg.H * 2}
     gpu_launches = st["kernel_launches"] * args.steps
 
     # resident-mode 32K number on the same weights (the second half of BASELINE's metric)
