@@ -81,6 +81,9 @@ typedef struct {
   int32_t gemm_impl;          /* 0: tcgen05/TMEM/TMA grouped GEMM (the product path).
                                  1: plain CUDA-core grouped GEMM kept for bring-up and for
                                  triaging the tensor-core kernel; same kernels around it. */
+  int32_t router_impl;        /* 0: router logits on the tensor cores (bf16 hi+lo split of the fp32
+                                 router weights, fp32 accumulate).  1: plain fp32 FMA kernel
+                                 (bring-up / triage). */
 } slp_moe_cfg;
 
 /* Host weight pointers.  Borrowed for the lifetime of the handle; the host copy stays

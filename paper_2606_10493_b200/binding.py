@@ -37,7 +37,8 @@ class _Cfg(C.Structure):
                 ("scoring", C.c_int32), ("norm_topk", C.c_int32), ("routed_scale", C.c_float),
                 ("max_tokens", C.c_int32), ("staging_slots", C.c_int32),
                 ("experts_per_launch", C.c_int32), ("skip_empty_experts", C.c_int32),
-                ("require_pinned", C.c_int32), ("gemm_impl", C.c_int32)]
+                ("require_pinned", C.c_int32), ("gemm_impl", C.c_int32),
+                ("router_impl", C.c_int32)]
 
 
 class _HostWeights(C.Structure):
@@ -119,7 +120,7 @@ class SlpMoeLayer:
     tensors, kept alive by this object because the library borrows the memory)."""
 
     def __init__(self, cfg, weights, *, max_tokens=None, device=0, staging_slots=0,
-                 experts_per_launch=0, skip_empty_experts=False, require_pinned=False, gemm_impl=0):
+                 experts_per_launch=0, skip_empty_experts=False, require_pinned=False, gemm_impl=0, router_impl=0):
         self._h = C.c_void_p()
         self.cfg = cfg
         self.weights = weights
@@ -131,7 +132,7 @@ class SlpMoeLayer:
                  routed_scale=cfg.routed_scale, max_tokens=self.max_tokens,
                  staging_slots=staging_slots, experts_per_launch=experts_per_launch,
                  skip_empty_experts=int(skip_empty_experts), require_pinned=int(require_pinned),
-                 gemm_impl=gemm_impl)
+                 gemm_impl=gemm_impl, router_impl=router_impl)
         w = weights
         self._arrays = {k: _ptr_array(w[k]) for k in ("gate_q", "gate_s", "up_q", "up_s", "down_q", "down_s")}
 

@@ -21,6 +21,7 @@
 #include "kernels_gemm_simt.cuh"
 #include "kernels_gemm_tc.cuh"
 #include "kernels_route.cuh"
+#include "kernels_router_tc.cuh"
 
 namespace {
 
@@ -95,6 +96,9 @@ struct slp_moe_layer {
   int residency = SLP_STREAMED;
 
   // resident device tensors
+  uint16_t* d_router_hl = nullptr;  // [2][Erows][H] bf16 hi / lo split of router_w (tensor-core router)
+  int Erows = 0;
+  CUtensorMap tm_rw{};
   float *d_router_w = nullptr, *d_bias = nullptr, *d_gate_s = nullptr, *d_up_s = nullptr, *d_down_s = nullptr;
   uint8_t* d_pool = nullptr;  // [1 + n_stage] slots; slot 0 = shared expert
   // workspace
@@ -284,8 +288,17 @@ slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t
   CU_TRY(cudaEventRecord(h->ev_t[0], s));
   // ---- a1 router ----
   {
-    dim3 grid((T + 63) / 64, (E + 63) / 64);
-    slp::router_logits_kernel<<<grid, 256, 0, s>>>(static_cast<const uint16_t*>(hidden), h->d_router_w, h->d_logits, T, H, E);
+    if (h->cfg.router_impl == 1) {
+      dim3 grid((T + 63) / 64, (E + 63) / 64);
+      slp::router_logits_kernel<<<grid, 256, 0, s>>>(static_cast<const uint16_t*>(hidden), h->d_router_w, h->d_logits, T, H, E);
+    } else {
+      CUtensorMap tm_x;
+      slp_status st = make_tmap_u8(&tm_x, const_cast<void*>(hidden), static_cast<uint64_t>(H) * 2, static_cast<uint64_t>(T));
+      if (st != SLP_OK) return st;
+      dim3 grid((T + slp::rtc::BM - 1) / slp::rtc::BM, (E + slp::rtc::BN - 1) / slp::rtc::BN);
+      slp::rtc::router_logits_tc_kernel<<<grid, slp::rtc::kThreads, slp::rtc::kSmemBytes, s>>>(tm_x, h->tm_rw, h->d_logits, T, H, E,
+                                                                                              h->Erows, h->d_err);
+    }
     const int warps = 8;
     const int blocks = (T + warps - 1) / warps;
     const float* bias = h->cfg.scoring == SLP_SCORE_SIGMOID_BIAS ? h->d_bias : nullptr;
@@ -418,6 +431,7 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
   if (cfg->scoring != SLP_SCORE_SIGMOID_BIAS && cfg->scoring != SLP_SCORE_SOFTMAX) return fail(SLP_ERR_INVALID_ARG, "unknown scoring %d", cfg->scoring);
   if (cfg->max_tokens <= 0) return fail(SLP_ERR_INVALID_ARG, "max_tokens must be positive");
   if (cfg->gemm_impl != 0 && cfg->gemm_impl != 1) return fail(SLP_ERR_INVALID_ARG, "gemm_impl must be 0 or 1");
+  if (cfg->router_impl != 0 && cfg->router_impl != 1) return fail(SLP_ERR_INVALID_ARG, "router_impl must be 0 or 1");
   int n_stage = cfg->staging_slots == 0 ? E : cfg->staging_slots;
   if (n_stage < 2 && E >= 2) return fail(SLP_ERR_INVALID_ARG, "staging_slots must be 0 or 2..n_experts");
   n_stage = std::min(n_stage, E);
@@ -501,6 +515,16 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
   const size_t sc_gu = static_cast<size_t>(h->kbI) * h->kbH, sc_d = static_cast<size_t>(h->kbH) * h->kbI;
   CU_OR_BAIL(cudaMalloc(&h->d_router_w, static_cast<size_t>(E) * H * sizeof(float)));
   CU_OR_BAIL(cudaMemcpy(h->d_router_w, w->router_w, static_cast<size_t>(E) * H * sizeof(float), cudaMemcpyHostToDevice));
+  {  // bf16 hi / lo split of the router weights for the tensor-core logits kernel
+    h->Erows = round_up(E, slp::rtc::BN);
+    const size_t hl_bytes = static_cast<size_t>(2) * h->Erows * H * sizeof(uint16_t);
+    CU_OR_BAIL(cudaMalloc(&h->d_router_hl, hl_bytes));
+    CU_OR_BAIL(cudaMemset(h->d_router_hl, 0, hl_bytes));
+    slp::rtc::split_router_w_kernel<<<h->num_sms * 4, 256>>>(h->d_router_w, h->d_router_hl, E, H, h->Erows);
+    CU_OR_BAIL(cudaGetLastError());
+    TRY_OR_BAIL(make_tmap_u8(&h->tm_rw, h->d_router_hl, static_cast<uint64_t>(H) * 2, static_cast<uint64_t>(2) * h->Erows));
+    CU_OR_BAIL(cudaFuncSetAttribute(slp::rtc::router_logits_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::rtc::kSmemBytes));
+  }
   CU_OR_BAIL(cudaMalloc(&h->d_bias, E * sizeof(float)));
   if (w->router_bias) CU_OR_BAIL(cudaMemcpy(h->d_bias, w->router_bias, E * sizeof(float), cudaMemcpyHostToDevice));
   else CU_OR_BAIL(cudaMemset(h->d_bias, 0, E * sizeof(float)));
@@ -634,7 +658,7 @@ slp_status slp_moe_layer_destroy(slp_moe_layer* h) {
   cudaSetDevice(h->cfg.device);
   cudaDeviceSynchronize();
   free_pool(h);
-  void* ptrs[] = {h->d_router_w, h->d_bias, h->d_gate_s, h->d_up_s, h->d_down_s, h->d_logits, h->d_w, h->d_xs, h->d_hs, h->d_idx,
+  void* ptrs[] = {h->d_router_hl, h->d_router_w, h->d_bias, h->d_gate_s, h->d_up_s, h->d_down_s, h->d_logits, h->d_w, h->d_xs, h->d_hs, h->d_idx,
                   h->d_counts, h->d_chunk, h->d_row_start, h->d_tile_start, h->d_tile_expert, h->d_pos, h->d_row_token, h->d_xq,
                   h->d_hq, h->d_y, h->d_err, h->d_e2e_in, h->d_e2e_out};
   for (void* p : ptrs)

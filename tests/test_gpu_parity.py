@@ -117,6 +117,31 @@ def test_layer_parity_tcgen05(name, mode):
     check(name, mode, gemm_impl=0)
 
 
+@pytest.mark.parametrize("name", list(CASES))
+@pytest.mark.parametrize("router_impl", [0, 1])
+def test_router_logits_error(name, router_impl):
+    """Router logits (SLP_BUF_LOGITS) against the fp64 product.  The tensor-core router splits the
+    fp32 weights into bf16 hi + lo (kernels_router_tc.cuh); its logit error must stay a decade
+    below the 1e-4 near-tie allowance on the selection scores (|d sigmoid| <= |d logit| / 4)."""
+    cfg, W, hidden, ref = problem(name)
+    layer = SlpMoeLayer(cfg, W, device=0, router_impl=router_impl)
+    try:
+        layer.set_residency("resident")
+        layer.prefill(hidden.cuda())
+        torch.cuda.synchronize()
+        logits = layer.debug_buffer("logits", np.float32).reshape(cfg.T, cfg.E)
+        idx, w, _ = layer.debug_routing(cfg.T)
+    finally:
+        layer.close()
+    x = hidden.to(torch.float64).numpy()
+    exact = x @ W["router_w"].to(torch.float64).numpy().T
+    err = np.abs(logits - exact).max()
+    print(name, "router_impl", router_impl, "max |logit error|", err)
+    assert err < 4e-5, err
+    r = compare_routing(idx, w, ref["route"])
+    assert r["passed"], r
+
+
 @pytest.mark.parametrize("kw", [dict(staging_slots=2, experts_per_launch=1),
                                 dict(staging_slots=8, experts_per_launch=4),
                                 dict(staging_slots=4, experts_per_launch=2, skip_empty_experts=True),
