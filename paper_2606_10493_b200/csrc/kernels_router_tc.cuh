@@ -85,7 +85,7 @@ router_logits_tc_kernel(const __grid_constant__ CUtensorMap tm_x, const __grid_c
     uint32_t phase = 0;
     for (int kb = 0; kb < num_kb; ++kb) {
       ptx::mbar_wait(&sh->empty[stage], phase ^ 1, dead, err, 11);
-      if (lane == 0) {
+      if (ptx::elect_one()) {
         uint8_t* sa = smem + stage * kStageBytes;
         uint8_t* sb = sa + kABytes;
         ptx::mbar_arrive_expect_tx(&sh->full[stage], kABytes + 2 * nbox * kBoxBytes);
@@ -105,7 +105,7 @@ router_logits_tc_kernel(const __grid_constant__ CUtensorMap tm_x, const __grid_c
     for (int kb = 0; kb < num_kb; ++kb) {
       ptx::mbar_wait(&sh->full[stage], phase, dead, err, 12);
       ptx::tc_fence_after();
-      if (lane == 0) {
+      if (ptx::elect_one()) {
         const uint8_t* sa = smem + stage * kStageBytes;
         const uint64_t adesc = ptx::umma_desc_k128(sa);
         const uint64_t hdesc = ptx::umma_desc_k128(sa + kABytes);

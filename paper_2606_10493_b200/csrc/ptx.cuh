@@ -43,17 +43,24 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
   return ok != 0;
 }
 
-// Bounded wait: every pipeline wait in the kernels goes through this.  If a wait exceeds
-// `kWatchdogCycles` the CTA-wide `dead` flag (shared) is raised, a code is left in `*err`
-// (global) and all later waits in the CTA fall through, so a protocol bug ends the kernel with
-// an error status instead of hanging the GPU.
+// Bounded wait: every pipeline wait in the kernels goes through this.  The fast path is a tight
+// try_wait loop (the instruction itself suspends the thread for a hardware-defined interval, so it
+// is not a hot spin); every 256 failed probes the slow path checks the CTA-wide `dead` flag and the
+// watchdog.  If a wait exceeds `kWatchdogCycles` the flag is raised, a code is left in `*err`
+// (global) and all later waits in the CTA fall through, so a protocol bug ends the kernel with an
+// error status instead of hanging the GPU.
 constexpr long long kWatchdogCycles = 4000000000LL;  // ~2 s at 1.9 GHz
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity, volatile int* dead, int* err, int code) {
   if (mbar_try_wait(bar, parity)) return;
-  long long t0 = clock64();
-  while (!mbar_try_wait(bar, parity)) {
+  long long t0 = 0;
+  for (;;) {
+#pragma unroll 1
+    for (int i = 0; i < 256; ++i)
+      if (mbar_try_wait(bar, parity)) return;
     if (*dead) return;
-    if (clock64() - t0 > kWatchdogCycles) {
+    const long long now = clock64();
+    if (t0 == 0) t0 = now;
+    if (now - t0 > kWatchdogCycles) {
       *dead = 1;
       atomicCAS(err, 0, code);
       return;
@@ -143,6 +150,21 @@ __device__ __forceinline__ void tmem_ld_wait16(uint32_t (&v)[16]) {
                  "+r"(v[8]), "+r"(v[9]), "+r"(v[10]), "+r"(v[11]), "+r"(v[12]), "+r"(v[13]), "+r"(v[14]), "+r"(v[15])
                :: "memory");
 }
+
+// Empty statement that reads and "writes" 16 registers: placed after the issue of the next
+// tcgen05.ld it keeps `v` live across that issue, so the two loads in flight get distinct registers
+// (asm volatile statements are not reordered against each other).
+__device__ __forceinline__ void keep16(uint32_t (&v)[16]) {
+  asm volatile(""
+               : "+r"(v[0]), "+r"(v[1]), "+r"(v[2]), "+r"(v[3]), "+r"(v[4]), "+r"(v[5]), "+r"(v[6]), "+r"(v[7]),
+                 "+r"(v[8]), "+r"(v[9]), "+r"(v[10]), "+r"(v[11]), "+r"(v[12]), "+r"(v[13]), "+r"(v[14]), "+r"(v[15]));
+}
+
+// Register re-balancing between warpgroups (all 128 threads of a warpgroup must execute it).
+template <int kRegs>
+__device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegs)); }
+template <int kRegs>
+__device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegs)); }
 
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");

@@ -63,13 +63,13 @@ EncodeTiledFn get_encode_fn() {
   return fn;
 }
 
-// 2D uint8 tensor [rows, inner] (row stride = inner bytes), box 128 B x 128 rows, 128B swizzle.
-slp_status make_tmap_u8(CUtensorMap* tm, void* base, uint64_t inner, uint64_t rows) {
+// 2D uint8 tensor [rows, inner] (row stride = inner bytes), box 128 B x box_rows rows, 128B swizzle.
+slp_status make_tmap_u8(CUtensorMap* tm, void* base, uint64_t inner, uint64_t rows, uint32_t box_rows = 128) {
   EncodeTiledFn fn = get_encode_fn();
   if (!fn) return fail(SLP_ERR_CUDA, "cuTensorMapEncodeTiled not available from the driver");
   cuuint64_t dims[2] = {inner, rows};
   cuuint64_t strides[1] = {inner};
-  cuuint32_t box[2] = {128, 128};
+  cuuint32_t box[2] = {128, box_rows};
   cuuint32_t estr[2] = {1, 1};
   CUresult r = fn(tm, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                   CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
@@ -157,9 +157,9 @@ slp_status alloc_pool(L* h, int n_stage, int epl) {
   } else {
     CU_TRY(cudaMemset(h->d_pool, 0, h->slot_bytes));
   }
-  slp_status st = make_tmap_u8(&h->tm_wgu, h->d_pool, h->H, static_cast<uint64_t>(1 + n_stage) * 3 * h->I);
+  slp_status st = make_tmap_u8(&h->tm_wgu, h->d_pool, h->H, static_cast<uint64_t>(1 + n_stage) * 3 * h->I, slp::tc::kBoxRows);
   if (st != SLP_OK) return st;
-  st = make_tmap_u8(&h->tm_wd, h->d_pool, h->I, static_cast<uint64_t>(1 + n_stage) * 3 * h->H);
+  st = make_tmap_u8(&h->tm_wd, h->d_pool, h->I, static_cast<uint64_t>(1 + n_stage) * 3 * h->H, slp::tc::kBoxRows);
   if (st != SLP_OK) return st;
   const int n_groups = (n_stage + epl - 1) / epl;
   h->ev_ready.resize(n_groups);
