@@ -262,6 +262,8 @@ def main():
     roofline["ms_per_launch"] = gu_ms
     roofline["launches_per_step"] = st["timed_gemm_pairs"]
     roofline["down_ms_per_launch"] = dn_ms
+    roofline["sm_mhz_during_kernel"] = st["sm_mhz_gateup"]
+    roofline["down_sm_mhz_during_kernel"] = st["sm_mhz_down"]
 
     extra = {"tflops_per_call": flops_call / (ms * 1e-3) / 1e12,
              "fp8_peak_nominal_tflops": 4500.0, "frac_of_nominal_fp8": flops_call / (ms * 1e-3) / 4.5e15,

@@ -78,9 +78,11 @@ typedef struct {
                                  prefill).  0: paper-faithful fixed order, every expert copied. */
   int32_t require_pinned;     /* 1: create fails with SLP_ERR_NOT_PINNED if a weight buffer is
                                  pageable.  0: create pins it with cudaHostRegister. */
-  int32_t gemm_impl;          /* 0: tcgen05/TMEM/TMA grouped GEMM (the product path).
+  int32_t gemm_impl;          /* 0: tcgen05/TMEM/TMA grouped GEMM, cta_group::2 MMA over clusters of two
+                                    CTAs (the product path).
                                  1: plain CUDA-core grouped GEMM kept for bring-up and for
-                                 triaging the tensor-core kernel; same kernels around it. */
+                                    triaging the tensor-core kernels; same kernels around it.
+                                 2: the one-CTA-per-tile variant of the tcgen05 kernel (triage). */
   int32_t router_impl;        /* 0: router logits on the tensor cores (bf16 hi+lo split of the fp32
                                  router weights, fp32 accumulate).  1: plain fp32 FMA kernel
                                  (bring-up / triage). */
@@ -126,6 +128,8 @@ typedef struct {
   int32_t timed_gemm_pairs;   /* gate/up + down launch pairs bracketed by CUDA events on the caller's stream */
   float ms_gateup_sum;        /* sum over those launches of the gate/up (+SwiGLU+requant) kernel time */
   float ms_down_sum;          /* same for the down kernel */
+  float sm_mhz_gateup;        /* average SM clock during the gate/up launches (clock64 / globaltimer of CTA 0) */
+  float sm_mhz_down;          /* same for the down launches */
 } slp_moe_stats;
 
 /* Buffers readable through slp_moe_debug_buffer (parity / evidence; layouts in DESIGN.md §5). */

@@ -57,7 +57,8 @@ class Stats(C.Structure):
                 ("bytes_copied", C.c_int64), ("ms_total", C.c_float), ("ms_copy_span", C.c_float),
                 ("ms_route", C.c_float), ("ms_experts", C.c_float), ("ms_combine", C.c_float),
                 ("gemm_launches", C.c_int32), ("kernel_launches", C.c_int32), ("m_tiles", C.c_int32),
-                ("timed_gemm_pairs", C.c_int32), ("ms_gateup_sum", C.c_float), ("ms_down_sum", C.c_float)]
+                ("timed_gemm_pairs", C.c_int32), ("ms_gateup_sum", C.c_float), ("ms_down_sum", C.c_float),
+                ("sm_mhz_gateup", C.c_float), ("sm_mhz_down", C.c_float)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_ if n != "struct_size"}

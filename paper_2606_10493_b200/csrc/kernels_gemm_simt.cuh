@@ -17,6 +17,9 @@ struct GemmArgs {
   const int32_t* tile_start;   // [E+2]
   const int32_t* row_start;    // [E+2]
   const int32_t* counts;       // [E]
+  const int4* tile_info;       // [tiles] {expert, first workspace row, valid rows, tile index inside the expert}
+  const int32_t* pair_start;   // [E+2] prefix of ceil(m tiles / 2) per expert (CTA-pair GEMM work items)
+  const int32_t* pair_expert;  // [pairs] expert of each pair of 128-row tiles
   int e_begin, e_end;          // experts covered by this launch: [e_begin, e_end), E = shared
   int E, T;
   int n_stage;                 // slot of routed expert e is 1 + e % n_stage; shared expert: slot 0
@@ -35,6 +38,8 @@ struct GemmArgs {
   int hs_stride;
   float* y;                    // [rows, H] fp32
   int* err;
+  unsigned long long* clk;     // [4] {SM cycles, ns} of CTA 0 summed over gate/up launches, then over down launches
+  int dbg;                     // timing experiments only (SLP_DBG env): 1 skip promotion math, 2 MMA ignores tmem_empty
 };
 
 __device__ __forceinline__ int slot_of(const GemmArgs& g, int e) { return e == g.E ? 0 : 1 + e % g.n_stage; }

@@ -41,28 +41,37 @@ namespace slp {
 namespace tc {
 
 constexpr int BM = 128, BN = 256, BK = 128, HN = 128;
-constexpr int kStages = 4;
-constexpr int kABytes = BM * BK, kBBytes = BN * BK, kStageBytes = kABytes + kBBytes;
 constexpr int kBoxRows = 64;  // rows per B TMA box
-#ifndef SLP_SPLIT_N
-#define SLP_SPLIT_N 0
-#endif
-constexpr bool kSplitN = SLP_SPLIT_N;  // issue each K block as two N = 128 MMA groups (finer TMEM hand-off, but A is read twice from smem)
 constexpr int kEpiWarps = 8;
 constexpr int kThreads = (kEpiWarps + 4) * 32;  // three warpgroups: 2 x promotion, 1 x {producer, MMA, 2 idle}
 constexpr int kTmemCols = 512;
 constexpr int kScratchBytes = kEpiWarps * 32 * 32 * 4;  // per-warp 32 x 32 fp32 transpose tile (mode 1) / amax exchange (mode 0)
-constexpr int kSmemBytes = kStages * kStageBytes + 1024 /*align*/ + 256 /*barriers*/ + kScratchBytes;
+constexpr int kMaxStages = 6;
 
+// kPair = false: one CTA per tile, A tile (16 KB) + whole B tile (32 KB) per stage, 4 stages.
+// kPair = true:  a cluster of two CTAs issues one cta_group::2 MMA with M = 256 (two 128-row tiles
+//                of the same expert) x N = 256; each CTA stages its own A tile and HALF of the B tile
+//                (16 KB + 16 KB per stage, 6 stages), which cuts the L2 -> SM operand traffic per MAC
+//                by a third (the 1-CTA kernel is L2-bandwidth bound, profiles/r1_gemm_baseline.md).
+template <bool kPair> struct Cfg {
+  static constexpr int kStages = kPair ? 6 : 4;
+  static constexpr int kABytes = BM * BK;
+  static constexpr int kBBytes = (kPair ? BN / 2 : BN) * BK;
+  static constexpr int kStageBytes = kABytes + kBBytes;
+  static constexpr int kSmemBytes = kStages * kStageBytes + 1024 /*align*/ + 256 /*barriers*/ + kScratchBytes;
+};
+
+// Barrier block behind the stage ring; the kernels address it through 32-bit shared addresses.
 struct Shared {
-  uint64_t full[kStages];
-  uint64_t empty[kStages];
-  uint64_t tmem_full[4];   // [buf * 2 + half]
-  uint64_t tmem_empty[4];
+  uint64_t full[kMaxStages];   // TMA -> MMA: stage landed (pair: lives in the leader CTA, fed by both CTAs' loads)
+  uint64_t empty[kMaxStages];  // MMA -> TMA: stage consumed (pair: multicast commit to both CTAs)
+  uint64_t tmem_full[2];       // MMA -> promotion: K block partial complete in TMEM buffer b
+  uint64_t tmem_empty[2];      // promotion -> MMA: buffer b read out (pair: 2 x kEpiWarps arrivals at the leader)
   uint32_t tmem_base;
   int dead;
 };
 static_assert(sizeof(Shared) <= 256, "barrier block");
+constexpr uint32_t kOffFull = 0, kOffEmpty = 8 * kMaxStages, kOffTmemFull = 16 * kMaxStages, kOffTmemEmpty = 16 * kMaxStages + 16;
 
 // silu(g) * u with the fast exponential and reciprocal (rel. error ~1e-6, three decades below the
 // e4m3 step that follows).
@@ -80,41 +89,80 @@ __device__ __forceinline__ uint32_t quant4_e4m3_r(float a, float b, float c, flo
   return static_cast<uint32_t>(lo) | (static_cast<uint32_t>(hi) << 16);
 }
 
-template <int kMode>
+template <int kMode, bool kPair>
 __global__ void __launch_bounds__(kThreads, 1)
-gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__ CUtensorMap tm_b, GemmArgs g) {
+gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__ CUtensorMap tm_b,
+               const __grid_constant__ CUtensorMap tm_y, GemmArgs g) {
+  using C = Cfg<kPair>;
+  constexpr int kStages = C::kStages, kABytes = C::kABytes, kStageBytes = C::kStageBytes;
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-  Shared* sh = reinterpret_cast<Shared*>(smem + kStages * kStageBytes);
-  uint8_t* scratch = smem + kStages * kStageBytes + 256;
+  uint8_t* scratch = smem + kStages * kStageBytes;  // 1024-aligned: per-warp staging for the Y TMA stores / amax exchange
+  Shared* sh = reinterpret_cast<Shared*>(scratch + kScratchBytes);
+  const uint32_t smem_a = ptx::launder_u32(ptx::smem_u32(smem));               // stage ring base (shared window address)
+  const uint32_t bar_a = ptx::launder_u32(smem_a + kStages * kStageBytes + kScratchBytes);  // barrier block base
+  const uint32_t rank = kPair ? ptx::cluster_ctarank() : 0u;                   // CTA of the pair; 0 = leader (issues the MMAs)
+  const uint32_t lead_bar = kPair ? ptx::launder_u32(ptx::mapa(bar_a, 0)) : bar_a;  // leader's barrier block (cluster address)
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  long long clk0 = 0;
+  unsigned long long ns0 = 0;
+  if (blockIdx.x == 0 && threadIdx.x == 0) {  // average SM clock of this launch (evidence for the power-capped regime)
+    clk0 = clock64();
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(ns0));
+  }
   const int K = kMode == 0 ? g.H : g.I;
   const int N = kMode == 0 ? g.I : g.H;
   const int num_kb = K / BK;
   const int n_tiles = kMode == 0 ? N / 128 : (N + BN - 1) / BN;
-  const int mt_begin = g.tile_start[g.e_begin], mt_end = g.tile_start[g.e_end];
-  const int total = (mt_end - mt_begin) * n_tiles;
+  // work items: (128-row tile | pair of tiles, N tile) over the experts of this launch
+  const int it_begin = kPair ? g.pair_start[g.e_begin] : g.tile_start[g.e_begin];
+  const int it_end = kPair ? g.pair_start[g.e_end] : g.tile_start[g.e_end];
+  const int total = (it_end - it_begin) * n_tiles;
+  const int w_first = kPair ? static_cast<int>(blockIdx.x >> 1) : static_cast<int>(blockIdx.x);
+  const int w_step = kPair ? static_cast<int>(gridDim.x >> 1) : static_cast<int>(gridDim.x);
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < kStages; ++i) { ptx::mbar_init(&sh->full[i], 1); ptx::mbar_init(&sh->empty[i], 1); }
-    for (int i = 0; i < 4; ++i) { ptx::mbar_init(&sh->tmem_full[i], 1); ptx::mbar_init(&sh->tmem_empty[i], kEpiWarps / 2); }
+    for (int i = 0; i < 2; ++i) { ptx::mbar_init(&sh->tmem_full[i], 1); ptx::mbar_init(&sh->tmem_empty[i], kPair ? 2 * kEpiWarps : kEpiWarps); }
     sh->dead = 0;
     ptx::fence_mbar_init();
   }
-  if (warp == kEpiWarps + 1) ptx::tmem_alloc<kTmemCols>(&sh->tmem_base);
+  if (warp == kEpiWarps + 1) {
+    if (kPair) ptx::tmem_alloc_2sm<kTmemCols>(&sh->tmem_base);
+    else ptx::tmem_alloc<kTmemCols>(&sh->tmem_base);
+  }
   if (warp == kEpiWarps && lane == 0) { ptx::prefetch_tmap(&tm_a); ptx::prefetch_tmap(&tm_b); }
   ptx::tc_fence_before();
   __syncthreads();
+  if (kPair) ptx::cluster_sync();  // the peer's barriers are initialised before anything remote touches them
   ptx::tc_fence_after();
   const uint32_t tmem_base = sh->tmem_base;
   volatile int* dead = &sh->dead;
 
-  // Work item w -> (m tile, n tile): n fastest, so the CTAs running together cover a few m tiles
-  // of one expert against all of its N tiles and share both operands through L2.
-  auto decode = [&](int w, int& mt, int& nt) {
-    mt = mt_begin + w / n_tiles;
-    nt = w % n_tiles;
+  // Work item w -> (expert, this CTA's 128-row tile inside the expert, N tile): n fastest, so the CTAs
+  // running together cover a few m tiles of one expert against all of its N tiles and share both
+  // operands through L2.  One 16-byte record per tile (written by permute_scan_kernel) replaces a
+  // chain of dependent loads.  Pair kernel: the second CTA of the last pair of an expert with an odd
+  // number of tiles gets nrows = 0 (it re-reads the previous tile and stores nothing).
+  struct Tile { int e, row0, nrows, nt; };
+  auto fetch = [&](int w) {
+    Tile t;
+    const int item = it_begin + w / n_tiles;
+    t.nt = w % n_tiles;
+    if (kPair) {
+      t.e = g.pair_expert[item];
+      const int mt_e = g.tile_start[t.e + 1] - g.tile_start[t.e];
+      int m_in_e = 2 * (item - g.pair_start[t.e]) + static_cast<int>(rank);
+      const bool valid = m_in_e < mt_e;
+      if (!valid) m_in_e = mt_e - 1;
+      t.row0 = g.row_start[t.e] + m_in_e * BM;
+      t.nrows = valid ? min(BM, rows_of(g, t.e) - m_in_e * BM) : 0;
+    } else {
+      const int4 ti = g.tile_info[item];
+      t.e = ti.x; t.row0 = ti.y; t.nrows = ti.z;
+    }
+    return t;
   };
 
   // Registers: 168 per thread at launch (384 threads); the producer / MMA warpgroup gives most of
@@ -122,83 +170,86 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
   if (warp >= kEpiWarps) {
    ptx::setmaxnreg_dec<40>();
    if (warp == kEpiWarps) {
-    // ===================== TMA producer =====================
-    int stage = 0;
-    uint32_t phase = 0;
-    for (int w = blockIdx.x; w < total; w += gridDim.x) {
-      int mt, nt;
-      decode(w, mt, nt);
-      const int e = g.tile_expert[mt];
-      const int row0 = g.row_start[e] + (mt - g.tile_start[e]) * BM;
-      const int slot = slot_of(g, e);
-      int brow[4];
-      if (kMode == 0) {
-        const int gate0 = slot * 3 * g.I + nt * 128;  // view [slots*3I, H]
-        brow[0] = gate0; brow[1] = gate0 + g.I; brow[2] = gate0 + 64; brow[3] = gate0 + g.I + 64;
-      } else {
-        const int down0 = slot * 3 * g.H + 2 * g.H + nt * BN;  // view [slots*3H, I]
-        brow[0] = down0; brow[1] = down0 + 64; brow[2] = down0 + 128; brow[3] = down0 + 192;
-      }
-      for (int kb = 0; kb < num_kb; ++kb) {
-        ptx::mbar_wait(&sh->empty[stage], phase ^ 1, dead, g.err, 1);
-        if (ptx::elect_one()) {
-          uint8_t* sa = smem + stage * kStageBytes;
-          uint8_t* sb = sa + kABytes;
-          ptx::mbar_arrive_expect_tx(&sh->full[stage], kStageBytes);
-          ptx::tma_load_2d(sa, &tm_a, &sh->full[stage], kb * BK, row0);
-#pragma unroll
-          for (int b = 0; b < 4; ++b) ptx::tma_load_2d(sb + b * kBoxRows * BK, &tm_b, &sh->full[stage], kb * BK, brow[b]);
+    // ===================== TMA producer (one elected thread) =====================
+    if (ptx::elect_one()) {
+      int stage = 0;
+      uint32_t phase = 0;
+      Tile nx = fetch(min(w_first, max(total - 1, 0)));
+      for (int w = w_first; w < total; w += w_step) {
+        const Tile cur = nx;
+        if (w + w_step < total) nx = fetch(w + w_step);  // next tile's record is in flight during this tile's loads
+        const int e = cur.e, nt = cur.nt, row0 = cur.row0;
+        const int slot = slot_of(g, e);
+        constexpr int kBoxes = kPair ? 2 : 4;
+        int brow[kBoxes];
+        if (kMode == 0) {
+          const int gate0 = slot * 3 * g.I + nt * 128;  // view [slots*3I, H]
+          if (kPair) { brow[0] = gate0 + 64 * rank; brow[1] = gate0 + g.I + 64 * rank; }
+          else { brow[0] = gate0; brow[1] = gate0 + g.I; brow[2 % kBoxes] = gate0 + 64; brow[3 % kBoxes] = gate0 + g.I + 64; }
+        } else {
+          const int down0 = slot * 3 * g.H + 2 * g.H + nt * BN;  // view [slots*3H, I]
+          if (kPair) { brow[0] = down0 + 128 * rank; brow[1] = brow[0] + 64; }
+          else { brow[0] = down0; brow[1] = down0 + 64; brow[2 % kBoxes] = down0 + 128; brow[3 % kBoxes] = down0 + 192; }
         }
-        __syncwarp();
-        if (++stage == kStages) { stage = 0; phase ^= 1; }
+        for (int kb = 0; kb < num_kb; ++kb) {
+          ptx::mbar_wait_a(bar_a + kOffEmpty + 8 * stage, phase ^ 1, dead, g.err, 1);
+          const uint32_t sa = smem_a + stage * kStageBytes, sb = sa + kABytes;
+          if (g.dbg & 8) {  // timing experiment: no loads, the MMA runs on stale shared memory
+            if (rank == 0) ptx::mbar_arrive_a(bar_a + kOffFull + 8 * stage);
+          } else if (kPair && (g.dbg & 16)) {  // timing experiment: plain TMA on a local barrier
+            const uint32_t fb = bar_a + kOffFull + 8 * stage;
+            ptx::mbar_arrive_expect_tx_a(fb, kStageBytes);
+            ptx::tma_load_2d_a(sa, &tm_a, fb, kb * BK, row0);
+#pragma unroll
+            for (int b = 0; b < kBoxes; ++b) ptx::tma_load_2d_a(sb + b * kBoxRows * BK, &tm_b, fb, kb * BK, brow[b]);
+          } else if (kPair) {
+            const uint32_t fb = lead_bar + kOffFull + 8 * stage;  // both CTAs' bytes complete on the leader's barrier
+            if (rank == 0) ptx::mbar_arrive_expect_tx_a(bar_a + kOffFull + 8 * stage, 2 * kStageBytes);
+            ptx::tma_load_2d_2sm(sa, &tm_a, fb, kb * BK, row0);
+#pragma unroll
+            for (int b = 0; b < kBoxes; ++b) ptx::tma_load_2d_2sm(sb + b * kBoxRows * BK, &tm_b, fb, kb * BK, brow[b]);
+          } else {
+            const uint32_t fb = bar_a + kOffFull + 8 * stage;
+            ptx::mbar_arrive_expect_tx_a(fb, kStageBytes);
+            ptx::tma_load_2d_a(sa, &tm_a, fb, kb * BK, row0);
+#pragma unroll
+            for (int b = 0; b < kBoxes; ++b) ptx::tma_load_2d_a(sb + b * kBoxRows * BK, &tm_b, fb, kb * BK, brow[b]);
+          }
+          if (++stage == kStages) { stage = 0; phase ^= 1; }
+        }
       }
     }
-  } else if (warp == kEpiWarps + 1) {
-    // ===================== MMA issuer =====================
-    constexpr uint32_t idesc_half = ptx::umma_idesc_e4m3_f32(BM, HN), idesc_full = ptx::umma_idesc_e4m3_f32(BM, BN);
-    int stage = 0;
-    uint32_t phase = 0;
-    uint32_t it = 0;  // running K-block counter: TMEM buffer = it & 1
-    for (int w = blockIdx.x; w < total; w += gridDim.x) {
-      for (int kb = 0; kb < num_kb; ++kb, ++it) {
-        const uint32_t buf = it & 1, tph = ((it >> 1) & 1) ^ 1;
-        ptx::mbar_wait(&sh->full[stage], phase, dead, g.err, 3);
-        if (kSplitN) {
-#pragma unroll
-          for (int half = 0; half < 2; ++half) {
-            ptx::mbar_wait(&sh->tmem_empty[buf * 2 + half], tph, dead, g.err, 2);
-            ptx::tc_fence_after();
-            if (ptx::elect_one()) {
-              const uint8_t* sa = smem + stage * kStageBytes;
-              const uint64_t adesc = ptx::umma_desc_k128(sa);
-              const uint64_t bdesc = ptx::umma_desc_k128(sa + kABytes + half * HN * BK);
-              const uint32_t d = tmem_base + buf * BN + half * HN;
-#pragma unroll
-              for (int k4 = 0; k4 < BK / 32; ++k4)  // UMMA_K = 32 for 8-bit operands: +32 B per step
-                ptx::umma_f8(d, adesc + 2 * k4, bdesc + 2 * k4, idesc_half, k4 > 0);
-              if (half == 1) ptx::umma_commit(&sh->empty[stage]);   // smem stage reusable once these MMAs retire
-              ptx::umma_commit(&sh->tmem_full[buf * 2 + half]);     // this half of the K block's partial is complete
-            }
-            __syncwarp();
-          }
-        } else {
-          ptx::mbar_wait(&sh->tmem_empty[buf * 2], tph, dead, g.err, 2);
-          ptx::mbar_wait(&sh->tmem_empty[buf * 2 + 1], tph, dead, g.err, 2);
+   } else if (warp == kEpiWarps + 1) {
+    // ===================== MMA issuer (one elected thread; pair: leader CTA only) =====================
+    if (rank == 0 && ptx::elect_one()) {
+      constexpr uint32_t idesc = ptx::umma_idesc_e4m3_f32(kPair ? 2 * BM : BM, BN);
+      const uint64_t adesc0 = ptx::umma_desc_k128_a(smem_a), bdesc0 = ptx::umma_desc_k128_a(smem_a + kABytes);
+      int stage = 0;
+      uint32_t phase = 0;
+      uint32_t it = 0;  // running K-block counter: TMEM buffer = it & 1
+      for (int w = w_first; w < total; w += w_step) {
+        for (int kb = 0; kb < num_kb; ++kb, ++it) {
+          const uint32_t buf = it & 1, tph = ((it >> 1) & 1) ^ 1;
+          ptx::mbar_wait_a(bar_a + kOffFull + 8 * stage, phase, dead, g.err, 3);    // operands landed (usually long ago)
+          ptx::mbar_wait_a(bar_a + kOffTmemEmpty + 8 * buf, tph, dead, g.err, 2);   // the critical hand-off: issue right after it
           ptx::tc_fence_after();
-          if (ptx::elect_one()) {
-            const uint8_t* sa = smem + stage * kStageBytes;
-            const uint64_t adesc = ptx::umma_desc_k128(sa);
-            const uint64_t bdesc = ptx::umma_desc_k128(sa + kABytes);
-            const uint32_t d = tmem_base + buf * BN;
+          const uint64_t so = static_cast<uint64_t>((stage * kStageBytes) >> 4);
+          const uint32_t d = tmem_base + buf * BN;
 #pragma unroll
-            for (int k4 = 0; k4 < BK / 32; ++k4) ptx::umma_f8(d, adesc + 2 * k4, bdesc + 2 * k4, idesc_full, k4 > 0);
-            ptx::umma_commit(&sh->empty[stage]);
-            ptx::umma_commit(&sh->tmem_full[buf * 2]);
-            ptx::umma_commit(&sh->tmem_full[buf * 2 + 1]);
+          for (int k4 = 0; k4 < BK / 32; ++k4) {  // UMMA_K = 32 for 8-bit operands: +32 B per step
+            if (g.dbg & 4) break;
+            if (kPair) ptx::umma_f8_2sm(d, adesc0 + so + 2 * k4, bdesc0 + so + 2 * k4, idesc, k4 > 0);
+            else ptx::umma_f8(d, adesc0 + so + 2 * k4, bdesc0 + so + 2 * k4, idesc, k4 > 0);
           }
-          __syncwarp();
+          if (kPair) {
+            ptx::umma_commit_2sm_mc(bar_a + kOffTmemFull + 8 * buf, 3);  // both CTAs' halves of the partial are complete
+            ptx::umma_commit_2sm_mc(bar_a + kOffEmpty + 8 * stage, 3);   // both CTAs' stages reusable once these MMAs retire
+          } else {
+            ptx::umma_commit_a(bar_a + kOffTmemFull + 8 * buf);
+            ptx::umma_commit_a(bar_a + kOffEmpty + 8 * stage);
+          }
+          if (++stage == kStages) { stage = 0; phase ^= 1; }
         }
-        if (++stage == kStages) { stage = 0; phase ^= 1; }
       }
     }
    }
@@ -207,62 +258,86 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
     ptx::setmaxnreg_inc<232>();
     const int q = warp & 3, half = warp >> 2;
     const int r_in_tile = q * 32 + lane;
-    const uint32_t lane_addr = static_cast<uint32_t>(q * 32) << 16;
+    const uint32_t tm_lane = ptx::launder_u32(tmem_base + (static_cast<uint32_t>(q * 32) << 16) + half * HN);
     uint32_t it = 0;
     int tile_parity = 0;
-    for (int w = blockIdx.x; w < total; w += gridDim.x, tile_parity ^= 1) {
-      int mt, nt;
-      decode(w, mt, nt);
-      const int e = g.tile_expert[mt];
-      const int m_in_e = mt - g.tile_start[e];
-      const int row0 = g.row_start[e] + m_in_e * BM;
-      const int nrows = min(BM, rows_of(g, e) - m_in_e * BM);
-      const size_t row = static_cast<size_t>(row0 + r_in_tile);
-      const bool row_ok = r_in_tile < nrows;
-      const float* as_ptr = g.a_s + row * g.a_s_stride;  // padded to a multiple of 4 floats, 16-byte aligned
+    const uint32_t te_a = lead_bar + kOffTmemEmpty;  // pair: the leader's barrier (cluster address)
+    // Per-tile scale pointers; the first loads of a tile are issued before the previous tile's epilogue.
+    const float *as_ptr = nullptr, *ws0 = nullptr, *ws1 = nullptr;
+    bool row_ok = false;
+    float4 xs_nxt = make_float4(0.f, 0.f, 0.f, 0.f);
+    float w0_nxt = 0.f, w1_nxt = 0.f;
+    auto open_tile = [&](const Tile& t) {
+      row_ok = r_in_tile < t.nrows;
+      as_ptr = g.a_s + static_cast<size_t>(t.row0 + r_in_tile) * g.a_s_stride;  // padded to a multiple of 4 floats, 16-byte aligned
       // weight-scale rows of this thread's columns: chunks 0-3 use ws0, chunks 4-7 use ws1
-      const float *ws0, *ws1;
       if (kMode == 0) {
-        const size_t o = (static_cast<size_t>(e) * (g.I / 128) + nt) * num_kb;
+        const size_t o = (static_cast<size_t>(t.e) * (g.I / 128) + t.nt) * num_kb;
         ws0 = g.gate_s + o;
         ws1 = g.up_s + o;
       } else {
-        const int nb = min(nt * 2 + half, g.H / 128 - 1);
-        ws0 = g.down_s + (static_cast<size_t>(e) * (g.H / 128) + nb) * num_kb;
+        const int nb = min(t.nt * 2 + half, g.H / 128 - 1);
+        ws0 = g.down_s + (static_cast<size_t>(t.e) * (g.H / 128) + nb) * num_kb;
         ws1 = ws0;
       }
-      float acc[128];
-#pragma unroll
-      for (int i = 0; i < 128; ++i) acc[i] = 0.f;
-
       // Scales are fetched far ahead of use: the row's activation scales four K blocks at a time
       // (one 16-byte load), the weight scales 32 K blocks at a time, one per lane, broadcast by shuffle.
-      float4 xs_nxt = row_ok ? *reinterpret_cast<const float4*>(as_ptr) : make_float4(0.f, 0.f, 0.f, 0.f);
-      float w0_nxt = lane < num_kb ? ws0[lane] : 0.f, w1_nxt = lane < num_kb ? ws1[lane] : 0.f;
-      float w0_cur = 0.f, w1_cur = 0.f;
-      for (int kb4 = 0; kb4 < num_kb; kb4 += 4) {
-        const float4 xs_cur = xs_nxt;
-        if (kb4 + 4 < num_kb && row_ok) xs_nxt = *reinterpret_cast<const float4*>(as_ptr + kb4 + 4);
-        if ((kb4 & 31) == 0) {
-          w0_cur = w0_nxt;
-          w1_cur = w1_nxt;
-          const int kn = kb4 + 32 + lane;
-          w0_nxt = kn < num_kb ? ws0[kn] : 0.f;
-          w1_nxt = kn < num_kb ? ws1[kn] : 0.f;
-        }
+      xs_nxt = row_ok ? *reinterpret_cast<const float4*>(as_ptr) : make_float4(0.f, 0.f, 0.f, 0.f);
+      w0_nxt = lane < num_kb ? ws0[lane] : 0.f;
+      w1_nxt = (kMode == 0 && lane < num_kb) ? ws1[lane] : 0.f;
+    };
+    Tile nx = fetch(min(w_first, max(total - 1, 0)));
+    if (w_first < total) open_tile(nx);
+    for (int w = w_first; w < total; w += w_step, tile_parity ^= 1) {
+      const Tile cur = nx;
+      const bool has_next = w + w_step < total;
+      if (has_next) nx = fetch(w + w_step);  // record in flight during the K loop
+      const int nt = cur.nt, row0 = cur.row0, nrows = cur.nrows;
+      const size_t row = static_cast<size_t>(row0 + r_in_tile);
+      const bool row_ok_cur = row_ok;
+      uint64_t acc2[64];  // 128 fp32 accumulators as FFMA2 pairs
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const int kb = kb4 + j;
-          if (kb >= num_kb) break;
+      for (int i = 0; i < 64; ++i) acc2[i] = 0ull;
+
+      float w0_cur = 0.f, w1_cur = 0.f;
+      float4 xs_cur = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll 1
+      for (int kb = 0; kb < num_kb; ++kb) {
+        {
+          if ((kb & 3) == 0) {
+            xs_cur = xs_nxt;
+            if (kb + 4 < num_kb && row_ok) xs_nxt = *reinterpret_cast<const float4*>(as_ptr + kb + 4);
+            if ((kb & 31) == 0) {
+              w0_cur = w0_nxt;
+              w1_cur = w1_nxt;
+              const int kn = kb + 32 + lane;
+              w0_nxt = kn < num_kb ? ws0[kn] : 0.f;
+              w1_nxt = kn < num_kb ? ws1[kn] : 0.f;
+            }
+          }
+          const int j = kb & 3;
           const float sa = j == 0 ? xs_cur.x : j == 1 ? xs_cur.y : j == 2 ? xs_cur.z : xs_cur.w;
           const float sc0 = sa * __shfl_sync(0xFFFFFFFFu, w0_cur, kb & 31);
           const float sc1 = kMode == 0 ? sa * __shfl_sync(0xFFFFFFFFu, w1_cur, kb & 31) : sc0;
+          const uint64_t s20 = ptx::pack2(sc0, sc0), s21 = ptx::pack2(sc1, sc1);
           const uint32_t buf = it & 1;
-          ptx::mbar_wait(&sh->tmem_full[buf * 2 + half], (it >> 1) & 1, dead, g.err, 4);
+          ptx::mbar_wait_a(bar_a + kOffTmemFull + 8 * buf, (it >> 1) & 1, dead, g.err, 4);
           ptx::tc_fence_after();
-          const uint32_t tb = tmem_base + lane_addr + buf * BN + half * HN;
-          // 8 chunks of 16 columns, two register sets in flight
+          const uint32_t tb = tm_lane + buf * BN;
+          // 8 chunks of 16 columns, two register sets in flight; one FFMA2 per column pair
           uint32_t v0[16], v1[16];
+          if (g.dbg & 1) {
+            ptx::tc_fence_before();
+            __syncwarp();
+            if (lane == 0) {
+              if (kPair && (g.dbg & 32)) {  // timing experiment: only the leader's warps release the buffer (twice each, locally)
+                if (rank == 0) { ptx::mbar_arrive_a(bar_a + kOffTmemEmpty + 8 * buf); ptx::mbar_arrive_a(bar_a + kOffTmemEmpty + 8 * buf); }
+              } else if (kPair) ptx::mbar_arrive_cluster(te_a + 8 * buf);
+              else ptx::mbar_arrive_a(te_a + 8 * buf);
+            }
+            ++it;
+            continue;
+          }
           ptx::tmem_ld16(tb, v0);
 #pragma unroll
           for (int c = 0; c < 8; c += 2) {
@@ -270,27 +345,36 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
             ptx::tmem_ld16(tb + (c + 1) * 16, v1);
             ptx::keep16(v0);  // v0 stays live across the issue of the next load: distinct registers
             {
-              const float sc = (c < 4) ? sc0 : sc1;
+              const uint64_t s2 = (c < 4) ? s20 : s21;
 #pragma unroll
-              for (int i = 0; i < 16; ++i) acc[c * 16 + i] = fmaf(__uint_as_float(v0[i]), sc, acc[c * 16 + i]);
+              for (int i = 0; i < 16; i += 2) ptx::fma2(acc2[c * 8 + i / 2], v0[i], v0[i + 1], s2);
             }
             ptx::tmem_ld_wait16(v1);
             if (c + 2 < 8) {
               ptx::tmem_ld16(tb + (c + 2) * 16, v0);
               ptx::keep16(v1);
+            } else {
+              // the whole partial is in registers: hand the TMEM buffer back before the last FMAs
+              ptx::tc_fence_before();
+              __syncwarp();
+              if (lane == 0) {
+                if (kPair && rank != 0) ptx::mbar_arrive_cluster(te_a + 8 * buf);  // remote: the leader's barrier
+                else ptx::mbar_arrive_a(bar_a + kOffTmemEmpty + 8 * buf);
+              }
             }
             {
-              const float sc = (c + 1 < 4) ? sc0 : sc1;
+              const uint64_t s2 = (c + 1 < 4) ? s20 : s21;
 #pragma unroll
-              for (int i = 0; i < 16; ++i) acc[(c + 1) * 16 + i] = fmaf(__uint_as_float(v1[i]), sc, acc[(c + 1) * 16 + i]);
+              for (int i = 0; i < 16; i += 2) ptx::fma2(acc2[(c + 1) * 8 + i / 2], v1[i], v1[i + 1], s2);
             }
           }
-          ptx::tc_fence_before();
-          __syncwarp();
-          if (lane == 0) ptx::mbar_arrive(&sh->tmem_empty[buf * 2 + half]);
           ++it;
         }
       }
+      if (has_next) open_tile(nx);  // first scale loads of the next tile fly during this tile's epilogue
+      float acc[128];
+#pragma unroll
+      for (int i = 0; i < 64; ++i) ptx::unpack2(acc2[i], acc[2 * i], acc[2 * i + 1]);
 
       if (kMode == 0) {
         // h = silu(gate) * up over this thread's 64 channels; row amax over all 128 via smem
@@ -305,7 +389,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
         ptx::named_bar_sync(1, kEpiWarps * 32);
         amax = fmaxf(amax, ex[(half ^ 1) * BM + r_in_tile]);
         const float s = (amax == 0.f) ? 1.0f : __fdiv_rn(amax, 448.0f);
-        if (row_ok) {
+        if (row_ok_cur) {
           uint32_t pk[16];
           if (s > 1e-30f) {
             const float r = __frcp_rn(s);
@@ -321,36 +405,53 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
           if (half == 0) g.hs[row * g.hs_stride + nt] = s;
         }
       } else {
-        // Y tile: transpose 32 x 32 fp32 quarters through this warp's smem tile (16-byte chunks
-        // XOR-swizzled by row) and store whole 128-byte row segments.
+        // Y tile (fp32, so that the layer's only bf16 rounding is the one in the combine): each warp owns
+        // 32 rows x 128 columns and streams them out as eight 32 x 16 boxes through a two-deep staging
+        // ring in shared memory (64-byte rows, 64B swizzle: conflict-free st.shared.v4) with TMA stores,
+        // so the global writes drain asynchronously while the warp starts the next tile's K loop.
+        // Rows past the expert's count are padding rows of the workspace; whole 32-row groups past it
+        // are skipped.
         const int c0 = nt * BN + half * HN;
-        float4* st = reinterpret_cast<float4*>(scratch + warp * 4096);
-        if (c0 < g.H) {
+        if (c0 < g.H && q * 32 < nrows) {
+          const uint32_t stage_a = smem_a + kStages * kStageBytes + warp * 4096;  // 2 x 2 KB per warp
+          const uint32_t sw = static_cast<uint32_t>((lane >> 1) & 3);
 #pragma unroll
-          for (int qq = 0; qq < 4; ++qq) {
-#pragma unroll
-            for (int j = 0; j < 8; ++j)
-              st[lane * 8 + (j ^ (lane & 7))] = make_float4(acc[qq * 32 + j * 4], acc[qq * 32 + j * 4 + 1], acc[qq * 32 + j * 4 + 2], acc[qq * 32 + j * 4 + 3]);
+          for (int c = 0; c < 8; ++c) {
+            const uint32_t dst = stage_a + (c & 1) * 2048;
+            if (lane == 0) ptx::bulk_wait_group_read<1>();  // the box that used this buffer two chunks ago has been read out
             __syncwarp();
 #pragma unroll
-            for (int i = 0; i < 8; ++i) {
-              const int rr = i * 4 + (lane >> 3), jj = lane & 7;
-              const float4 v = st[rr * 8 + (jj ^ (rr & 7))];
-              if (q * 32 + rr < nrows)
-                *reinterpret_cast<float4*>(g.y + static_cast<size_t>(row0 + q * 32 + rr) * g.H + c0 + qq * 32 + jj * 4) = v;
+            for (int j = 0; j < 4; ++j) {
+              const uint32_t a = dst + lane * 64 + ((static_cast<uint32_t>(j) ^ sw) << 4);
+              asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(a), "f"(acc[c * 16 + j * 4]), "f"(acc[c * 16 + j * 4 + 1]),
+                           "f"(acc[c * 16 + j * 4 + 2]), "f"(acc[c * 16 + j * 4 + 3]) : "memory");
             }
+            ptx::fence_proxy_async_smem();
             __syncwarp();
+            if (lane == 0) {
+              ptx::tma_store_2d_a(&tm_y, dst, c0 + c * 16, row0 + q * 32);
+              ptx::bulk_commit_group();
+            }
           }
         }
       }
     }
+    if (kMode == 1 && lane == 0) ptx::bulk_wait_group_read<0>();  // staging memory must outlive the last stores
   }
 
   ptx::tc_fence_before();
   __syncthreads();
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    unsigned long long ns1;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(ns1));
+    atomicAdd(&g.clk[2 * kMode], static_cast<unsigned long long>(clock64() - clk0));
+    atomicAdd(&g.clk[2 * kMode + 1], ns1 - ns0);
+  }
+  if (kPair) ptx::cluster_sync();  // no CTA leaves while its peer can still signal its barriers or read its smem
   if (warp == kEpiWarps + 1) {
     ptx::tc_fence_after();
-    ptx::tmem_dealloc<kTmemCols>(tmem_base);
+    if (kPair) ptx::tmem_dealloc_2sm<kTmemCols>(tmem_base);
+    else ptx::tmem_dealloc<kTmemCols>(tmem_base);
   }
 }
 

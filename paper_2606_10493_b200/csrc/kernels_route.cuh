@@ -236,10 +236,13 @@ __global__ void __launch_bounds__(128) permute_hist_kernel(const int32_t* __rest
 
 __global__ void __launch_bounds__(512) permute_scan_kernel(int32_t* __restrict__ chunk_counts, int32_t* __restrict__ counts,
                                                            int32_t* __restrict__ row_start, int32_t* __restrict__ tile_start,
-                                                           int32_t* __restrict__ tile_expert, int n_chunks, int T, int E,
-                                                           int has_shared) {
+                                                           int32_t* __restrict__ tile_expert, int32_t* __restrict__ pair_start,
+                                                           int32_t* __restrict__ pair_expert, int4* __restrict__ tile_info,
+                                                           int n_chunks, int T, int E, int has_shared) {
   __shared__ int32_t s_cnt[kMaxExperts + 1];
   __shared__ int32_t s_tile[kMaxExperts + 2];
+  __shared__ int32_t s_row[kMaxExperts + 2];
+  __shared__ int32_t s_pair[kMaxExperts + 2];  // prefix of ceil(m tiles / 2): work items of the CTA-pair GEMM
   const int e = threadIdx.x;
   if (e < E) {
     int run = 0;
@@ -259,24 +262,38 @@ __global__ void __launch_bounds__(512) permute_scan_kernel(int32_t* __restrict__
   __syncthreads();
   if (threadIdx.x == 0) {
     const int Tpad = (T + 127) / 128 * 128;
-    int row = Tpad, tile = 0;
+    int row = Tpad, tile = 0, pair = 0;
     for (int i = 0; i < E; ++i) {
       row_start[i] = row;
+      s_row[i] = row;
       s_tile[i] = tile;
+      s_pair[i] = pair;
       int mt = (s_cnt[i] + 127) / 128;
       row += mt * 128;
       tile += mt;
+      pair += (mt + 1) / 2;
     }
     row_start[E] = 0;  // shared expert: the un-permuted rows
+    s_row[E] = 0;
+    s_cnt[E] = T;
     s_tile[E] = tile;
+    s_pair[E] = pair;
     tile += has_shared ? Tpad / 128 : 0;
+    pair += has_shared ? (Tpad / 128 + 1) / 2 : 0;
     s_tile[E + 1] = tile;
+    s_pair[E + 1] = pair;
     row_start[E + 1] = row;  // total rows in use
   }
   __syncthreads();
-  for (int i = threadIdx.x; i < E + 2; i += blockDim.x) tile_start[i] = s_tile[i];
-  for (int i = threadIdx.x; i <= E; i += blockDim.x)
-    for (int m = s_tile[i]; m < s_tile[i + 1]; ++m) tile_expert[m] = i;
+  for (int i = threadIdx.x; i < E + 2; i += blockDim.x) { tile_start[i] = s_tile[i]; pair_start[i] = s_pair[i]; }
+  for (int i = threadIdx.x; i <= E; i += blockDim.x) {
+    for (int m = s_tile[i]; m < s_tile[i + 1]; ++m) {
+      tile_expert[m] = i;
+      const int m_in_e = m - s_tile[i];  // one record per 128-row tile: {expert, first workspace row, valid rows, tile index in expert}
+      tile_info[m] = make_int4(i, s_row[i] + m_in_e * 128, min(128, s_cnt[i] - m_in_e * 128), m_in_e);
+    }
+    for (int m = s_pair[i]; m < s_pair[i + 1]; ++m) pair_expert[m] = i;
+  }
 }
 
 __global__ void __launch_bounds__(128) permute_place_kernel(const int32_t* __restrict__ idx, const int32_t* __restrict__ chunk_off,

@@ -12,6 +12,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <mutex>
 #include <new>
 #include <string>
@@ -77,6 +78,20 @@ slp_status make_tmap_u8(CUtensorMap* tm, void* base, uint64_t inner, uint64_t ro
   return SLP_OK;
 }
 
+// 2D fp32 tensor [rows, inner] for TMA stores of 16-column x 32-row boxes (64-byte rows, 64B swizzle).
+slp_status make_tmap_f32_store(CUtensorMap* tm, void* base, uint64_t inner, uint64_t rows) {
+  EncodeTiledFn fn = get_encode_fn();
+  if (!fn) return fail(SLP_ERR_CUDA, "cuTensorMapEncodeTiled not available from the driver");
+  cuuint64_t dims[2] = {inner, rows};
+  cuuint64_t strides[1] = {inner * 4};
+  cuuint32_t box[2] = {16, 32};
+  cuuint32_t estr[2] = {1, 1};
+  CUresult r = fn(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                  CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(SLP_ERR_CUDA, "cuTensorMapEncodeTiled (Y store) failed with CUresult %d", static_cast<int>(r));
+  return SLP_OK;
+}
+
 inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
 
 }  // namespace
@@ -104,15 +119,17 @@ struct slp_moe_layer {
   // workspace
   float *d_logits = nullptr, *d_w = nullptr, *d_xs = nullptr, *d_hs = nullptr;
   int32_t *d_idx = nullptr, *d_counts = nullptr, *d_chunk = nullptr, *d_row_start = nullptr, *d_tile_start = nullptr,
-          *d_tile_expert = nullptr, *d_pos = nullptr, *d_row_token = nullptr;
+          *d_tile_expert = nullptr, *d_pos = nullptr, *d_row_token = nullptr, *d_pair_start = nullptr, *d_pair_expert = nullptr;
+  int4* d_tile_info = nullptr;
   uint8_t *d_xq = nullptr, *d_hq = nullptr;
   float* d_y = nullptr;
   int* d_err = nullptr;
+  unsigned long long* d_clk = nullptr;
   void *d_e2e_in = nullptr, *d_e2e_out = nullptr;
   int32_t* h_counts = nullptr;  // pinned
   int* h_err = nullptr;         // pinned
 
-  CUtensorMap tm_xq{}, tm_hq{}, tm_wgu{}, tm_wd{};
+  CUtensorMap tm_xq{}, tm_hq{}, tm_wgu{}, tm_wd{}, tm_y{};
 
   cudaStream_t copy_stream = nullptr, own_stream = nullptr;
   std::vector<cudaEvent_t> ev_ready, ev_free;
@@ -212,6 +229,9 @@ slp::GemmArgs gemm_args(L* h, int mode, int e_begin, int e_end, int T) {
   g.tile_start = h->d_tile_start;
   g.row_start = h->d_row_start;
   g.counts = h->d_counts;
+  g.tile_info = h->d_tile_info;
+  g.pair_start = h->d_pair_start;
+  g.pair_expert = h->d_pair_expert;
   g.e_begin = e_begin;
   g.e_end = e_end;
   g.E = h->E;
@@ -231,6 +251,8 @@ slp::GemmArgs gemm_args(L* h, int mode, int e_begin, int e_end, int T) {
   g.hs_stride = h->hs_stride;
   g.y = h->d_y;
   g.err = h->d_err;
+  g.clk = h->d_clk;
+  { const char* d = getenv("SLP_DBG"); g.dbg = d ? atoi(d) : 0; }
   return g;
 }
 
@@ -245,13 +267,35 @@ slp_status launch_experts(L* h, cudaStream_t s, int e_begin, int e_end, int T, i
   } else {
     slp::GemmArgs g0 = gemm_args(h, 0, e_begin, e_end, T), g1 = gemm_args(h, 1, e_begin, e_end, T);
     const int nt0 = h->I / 128, nt1 = (h->H + 255) / 256;
-    const int grid0 = std::max(1, std::min(h->num_sms, max_tiles * nt0));
-    const int grid1 = std::max(1, std::min(h->num_sms, max_tiles * nt1));
     cudaEvent_t* ev = (h->ev_k_used + 3 <= static_cast<int>(h->ev_k.size())) ? &h->ev_k[h->ev_k_used] : nullptr;
     if (ev) cudaEventRecord(ev[0], s);
-    slp::tc::gemm_tc_kernel<0><<<grid0, slp::tc::kThreads, slp::tc::kSmemBytes, s>>>(h->tm_xq, h->tm_wgu, g0);
-    if (ev) cudaEventRecord(ev[1], s);
-    slp::tc::gemm_tc_kernel<1><<<grid1, slp::tc::kThreads, slp::tc::kSmemBytes, s>>>(h->tm_hq, h->tm_wd, g1);
+    if (h->cfg.gemm_impl == 2) {
+      // CTA-pair kernel: clusters of two CTAs, one per SM; a work item is a pair of 128-row tiles
+      namespace tc = slp::tc;
+      const int n_cl = h->num_sms / 2;
+      cudaLaunchAttribute attr[1];
+      attr[0].id = cudaLaunchAttributeClusterDimension;
+      attr[0].val.clusterDim.x = 2;
+      attr[0].val.clusterDim.y = 1;
+      attr[0].val.clusterDim.z = 1;
+      cudaLaunchConfig_t lc{};
+      lc.blockDim = dim3(tc::kThreads);
+      lc.dynamicSmemBytes = tc::Cfg<true>::kSmemBytes;
+      lc.stream = s;
+      lc.attrs = attr;
+      lc.numAttrs = 1;
+      lc.gridDim = dim3(2 * std::max(1, std::min(n_cl, max_tiles * nt0)));
+      CU_TRY(cudaLaunchKernelEx(&lc, tc::gemm_tc_kernel<0, true>, h->tm_xq, h->tm_wgu, h->tm_y, g0));
+      if (ev) cudaEventRecord(ev[1], s);
+      lc.gridDim = dim3(2 * std::max(1, std::min(n_cl, max_tiles * nt1)));
+      CU_TRY(cudaLaunchKernelEx(&lc, tc::gemm_tc_kernel<1, true>, h->tm_hq, h->tm_wd, h->tm_y, g1));
+    } else {
+      const int grid0 = std::max(1, std::min(h->num_sms, max_tiles * nt0));
+      const int grid1 = std::max(1, std::min(h->num_sms, max_tiles * nt1));
+      slp::tc::gemm_tc_kernel<0, false><<<grid0, slp::tc::kThreads, slp::tc::Cfg<false>::kSmemBytes, s>>>(h->tm_xq, h->tm_wgu, h->tm_y, g0);
+      if (ev) cudaEventRecord(ev[1], s);
+      slp::tc::gemm_tc_kernel<1, false><<<grid1, slp::tc::kThreads, slp::tc::Cfg<false>::kSmemBytes, s>>>(h->tm_hq, h->tm_wd, h->tm_y, g1);
+    }
     if (ev) {
       cudaEventRecord(ev[2], s);
       h->ev_k_used += 3;
@@ -285,6 +329,7 @@ slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t
   h->ev_k_used = 0;
   auto launched = [&](int n) { h->stats.kernel_launches += n; };
 
+  CU_TRY(cudaMemsetAsync(h->d_clk, 0, 4 * sizeof(unsigned long long), s));
   CU_TRY(cudaEventRecord(h->ev_t[0], s));
   // ---- a1 router ----
   {
@@ -321,7 +366,7 @@ slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t
     const size_t sm = static_cast<size_t>(wpb) * E * sizeof(int32_t);
     CU_TRY(cudaMemsetAsync(h->d_row_token, 0xFF, static_cast<size_t>(h->rows_max) * sizeof(int32_t), s));
     slp::permute_hist_kernel<<<blocks, wpb * 32, sm, s>>>(h->d_idx, h->d_chunk, T, k, E);
-    slp::permute_scan_kernel<<<1, 512, 0, s>>>(h->d_chunk, h->d_counts, h->d_row_start, h->d_tile_start, h->d_tile_expert, n_chunks, T,
+    slp::permute_scan_kernel<<<1, 512, 0, s>>>(h->d_chunk, h->d_counts, h->d_row_start, h->d_tile_start, h->d_tile_expert, h->d_pair_start, h->d_pair_expert, h->d_tile_info, n_chunks, T,
                                                E, shared ? 1 : 0);
     slp::permute_place_kernel<<<blocks, wpb * 32, sm, s>>>(h->d_idx, h->d_chunk, h->d_row_start, h->d_pos, h->d_row_token, T, k, E);
     launched(3);
@@ -430,7 +475,7 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
     return fail(SLP_ERR_UNSUPPORTED_SHAPE, "n_shared must be 0 or 1 with shared_intermediate == moe_intermediate");
   if (cfg->scoring != SLP_SCORE_SIGMOID_BIAS && cfg->scoring != SLP_SCORE_SOFTMAX) return fail(SLP_ERR_INVALID_ARG, "unknown scoring %d", cfg->scoring);
   if (cfg->max_tokens <= 0) return fail(SLP_ERR_INVALID_ARG, "max_tokens must be positive");
-  if (cfg->gemm_impl != 0 && cfg->gemm_impl != 1) return fail(SLP_ERR_INVALID_ARG, "gemm_impl must be 0 or 1");
+  if (cfg->gemm_impl < 0 || cfg->gemm_impl > 2) return fail(SLP_ERR_INVALID_ARG, "gemm_impl must be 0, 1 or 2");
   if (cfg->router_impl != 0 && cfg->router_impl != 1) return fail(SLP_ERR_INVALID_ARG, "router_impl must be 0 or 1");
   int n_stage = cfg->staging_slots == 0 ? E : cfg->staging_slots;
   if (n_stage < 2 && E >= 2) return fail(SLP_ERR_INVALID_ARG, "staging_slots must be 0 or 2..n_experts");
@@ -552,6 +597,9 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
   CU_OR_BAIL(cudaMalloc(&h->d_row_start, (E + 2) * sizeof(int32_t)));
   CU_OR_BAIL(cudaMalloc(&h->d_tile_start, (E + 2) * sizeof(int32_t)));
   CU_OR_BAIL(cudaMalloc(&h->d_tile_expert, static_cast<size_t>(h->tiles_max) * sizeof(int32_t)));
+  CU_OR_BAIL(cudaMalloc(&h->d_tile_info, static_cast<size_t>(h->tiles_max) * sizeof(int4)));
+  CU_OR_BAIL(cudaMalloc(&h->d_pair_start, (E + 2) * sizeof(int32_t)));
+  CU_OR_BAIL(cudaMalloc(&h->d_pair_expert, static_cast<size_t>(h->tiles_max) * sizeof(int32_t)));
   CU_OR_BAIL(cudaMalloc(&h->d_pos, Tm * k * sizeof(int32_t)));
   CU_OR_BAIL(cudaMalloc(&h->d_row_token, rows * sizeof(int32_t)));
   CU_OR_BAIL(cudaMalloc(&h->d_xq, rows * H));
@@ -559,6 +607,7 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
   CU_OR_BAIL(cudaMalloc(&h->d_hq, rows * I));
   CU_OR_BAIL(cudaMalloc(&h->d_hs, rows * h->hs_stride * sizeof(float)));
   CU_OR_BAIL(cudaMalloc(&h->d_y, rows * H * sizeof(float)));
+  CU_OR_BAIL(cudaMalloc(&h->d_clk, 4 * sizeof(unsigned long long)));
   CU_OR_BAIL(cudaMalloc(&h->d_err, sizeof(int)));
   CU_OR_BAIL(cudaMemset(h->d_err, 0, sizeof(int)));
   // padding rows are read by the tensor cores (their outputs are discarded): keep them finite
@@ -570,10 +619,13 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
 
   TRY_OR_BAIL(make_tmap_u8(&h->tm_xq, h->d_xq, H, rows));
   TRY_OR_BAIL(make_tmap_u8(&h->tm_hq, h->d_hq, I, rows));
+  TRY_OR_BAIL(make_tmap_f32_store(&h->tm_y, h->d_y, H, rows));
   TRY_OR_BAIL(alloc_pool(h, n_stage, epl));
 
-  CU_OR_BAIL(cudaFuncSetAttribute(slp::tc::gemm_tc_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::tc::kSmemBytes));
-  CU_OR_BAIL(cudaFuncSetAttribute(slp::tc::gemm_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::tc::kSmemBytes));
+  CU_OR_BAIL(cudaFuncSetAttribute(slp::tc::gemm_tc_kernel<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::tc::Cfg<true>::kSmemBytes));
+  CU_OR_BAIL(cudaFuncSetAttribute(slp::tc::gemm_tc_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::tc::Cfg<true>::kSmemBytes));
+  CU_OR_BAIL(cudaFuncSetAttribute(slp::tc::gemm_tc_kernel<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::tc::Cfg<false>::kSmemBytes));
+  CU_OR_BAIL(cudaFuncSetAttribute(slp::tc::gemm_tc_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::tc::Cfg<false>::kSmemBytes));
   CU_OR_BAIL(cudaDeviceSynchronize());
 #undef TRY_OR_BAIL
 #undef CU_OR_BAIL
@@ -659,8 +711,8 @@ slp_status slp_moe_layer_destroy(slp_moe_layer* h) {
   cudaDeviceSynchronize();
   free_pool(h);
   void* ptrs[] = {h->d_router_hl, h->d_router_w, h->d_bias, h->d_gate_s, h->d_up_s, h->d_down_s, h->d_logits, h->d_w, h->d_xs, h->d_hs, h->d_idx,
-                  h->d_counts, h->d_chunk, h->d_row_start, h->d_tile_start, h->d_tile_expert, h->d_pos, h->d_row_token, h->d_xq,
-                  h->d_hq, h->d_y, h->d_err, h->d_e2e_in, h->d_e2e_out};
+                  h->d_counts, h->d_chunk, h->d_row_start, h->d_tile_start, h->d_tile_expert, h->d_pair_start, h->d_pair_expert, h->d_tile_info, h->d_pos, h->d_row_token, h->d_xq,
+                  h->d_hq, h->d_y, h->d_err, h->d_clk, h->d_e2e_in, h->d_e2e_out};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   if (h->h_counts) cudaFreeHost(h->h_counts);
@@ -756,6 +808,10 @@ slp_status slp_moe_get_stats(slp_moe_layer* h, slp_moe_stats* stats) {
       h->stats.ms_gateup_sum += a;
       h->stats.ms_down_sum += b;
     }
+    unsigned long long clk[4] = {0, 0, 0, 0};
+    CU_TRY(cudaMemcpy(clk, h->d_clk, sizeof clk, cudaMemcpyDeviceToHost));
+    h->stats.sm_mhz_gateup = clk[1] ? static_cast<float>(1e3 * static_cast<double>(clk[0]) / static_cast<double>(clk[1])) : 0.f;
+    h->stats.sm_mhz_down = clk[3] ? static_cast<float>(1e3 * static_cast<double>(clk[2]) / static_cast<double>(clk[3])) : 0.f;
     int32_t ts[1] = {0};
     CU_TRY(cudaMemcpy(ts, h->d_tile_start + h->E + 1, sizeof(int32_t), cudaMemcpyDeviceToHost));
     h->stats.m_tiles = ts[0];
