@@ -39,7 +39,6 @@ struct GemmArgs {
   float* y;                    // [rows, H] fp32
   int* err;
   unsigned long long* clk;     // [4] {SM cycles, ns} of CTA 0 summed over gate/up launches, then over down launches
-  int dbg;                     // timing experiments only (SLP_DBG env): 1 skip promotion math, 2 MMA ignores tmem_empty
 };
 
 __device__ __forceinline__ int slot_of(const GemmArgs& g, int e) { return e == g.E ? 0 : 1 + e % g.n_stage; }

@@ -194,15 +194,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
         for (int kb = 0; kb < num_kb; ++kb) {
           ptx::mbar_wait_a(bar_a + kOffEmpty + 8 * stage, phase ^ 1, dead, g.err, 1);
           const uint32_t sa = smem_a + stage * kStageBytes, sb = sa + kABytes;
-          if (g.dbg & 8) {  // timing experiment: no loads, the MMA runs on stale shared memory
-            if (rank == 0) ptx::mbar_arrive_a(bar_a + kOffFull + 8 * stage);
-          } else if (kPair && (g.dbg & 16)) {  // timing experiment: plain TMA on a local barrier
-            const uint32_t fb = bar_a + kOffFull + 8 * stage;
-            ptx::mbar_arrive_expect_tx_a(fb, kStageBytes);
-            ptx::tma_load_2d_a(sa, &tm_a, fb, kb * BK, row0);
-#pragma unroll
-            for (int b = 0; b < kBoxes; ++b) ptx::tma_load_2d_a(sb + b * kBoxRows * BK, &tm_b, fb, kb * BK, brow[b]);
-          } else if (kPair) {
+          if (kPair) {
             const uint32_t fb = lead_bar + kOffFull + 8 * stage;  // both CTAs' bytes complete on the leader's barrier
             if (rank == 0) ptx::mbar_arrive_expect_tx_a(bar_a + kOffFull + 8 * stage, 2 * kStageBytes);
             ptx::tma_load_2d_2sm(sa, &tm_a, fb, kb * BK, row0);
@@ -237,7 +229,6 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
           const uint32_t d = tmem_base + buf * BN;
 #pragma unroll
           for (int k4 = 0; k4 < BK / 32; ++k4) {  // UMMA_K = 32 for 8-bit operands: +32 B per step
-            if (g.dbg & 4) break;
             if (kPair) ptx::umma_f8_2sm(d, adesc0 + so + 2 * k4, bdesc0 + so + 2 * k4, idesc, k4 > 0);
             else ptx::umma_f8(d, adesc0 + so + 2 * k4, bdesc0 + so + 2 * k4, idesc, k4 > 0);
           }
@@ -312,7 +303,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
               w1_cur = w1_nxt;
               const int kn = kb + 32 + lane;
               w0_nxt = kn < num_kb ? ws0[kn] : 0.f;
-              w1_nxt = kn < num_kb ? ws1[kn] : 0.f;
+              w1_nxt = (kMode == 0 && kn < num_kb) ? ws1[kn] : 0.f;
             }
           }
           const int j = kb & 3;
@@ -326,18 +317,6 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
           const uint32_t tb = tm_lane + buf * BN;
           // 8 chunks of 16 columns, two register sets in flight; one FFMA2 per column pair
           uint32_t v0[16], v1[16];
-          if (g.dbg & 1) {
-            ptx::tc_fence_before();
-            __syncwarp();
-            if (lane == 0) {
-              if (kPair && (g.dbg & 32)) {  // timing experiment: only the leader's warps release the buffer (twice each, locally)
-                if (rank == 0) { ptx::mbar_arrive_a(bar_a + kOffTmemEmpty + 8 * buf); ptx::mbar_arrive_a(bar_a + kOffTmemEmpty + 8 * buf); }
-              } else if (kPair) ptx::mbar_arrive_cluster(te_a + 8 * buf);
-              else ptx::mbar_arrive_a(te_a + 8 * buf);
-            }
-            ++it;
-            continue;
-          }
           ptx::tmem_ld16(tb, v0);
 #pragma unroll
           for (int c = 0; c < 8; c += 2) {
