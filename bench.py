@@ -36,6 +36,9 @@ WORKLOADS = {
     "cfg4_resident": (4, "resident"),
 }
 METRIC = "prefill tok/s per MoE layer (host-streamed FP8); resident FP8 TFLOP/s vs peak"
+# dram__bytes_read.sum + dram__bytes_write.sum of one gemm_tc_kernel<0> launch, from the committed ncu
+# --set full captures (profiles/r1_layer_ncu.md, profiles/r1_streamed_gemm_ncu.md); None = not captured.
+NCU_TRAFFIC_BYTES = {"cfg2_resident": 28.69e9, "cfg1_streamed": None}
 
 
 def load_peaks():
@@ -258,7 +261,9 @@ def main():
                     "achieved": gu_bytes / gu_time / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                     "peak_source": f"hbm copy {peaks['source']}"}
     roofline["frac"] = roofline["achieved"] / roofline["peak"]
-    roofline["traffic"] = None
+    roofline["traffic"] = NCU_TRAFFIC_BYTES.get(args.workload)
+    roofline["algorithmic_bytes_per_launch"] = gu_bytes / max(1, st["timed_gemm_pairs"])
+    roofline["algorithmic_flops_per_launch"] = gu_flops / max(1, st["timed_gemm_pairs"])
     roofline["ms_per_launch"] = gu_ms
     roofline["launches_per_step"] = st["timed_gemm_pairs"]
     roofline["down_ms_per_launch"] = dn_ms
@@ -327,7 +332,14 @@ def main():
                                      "tflops_per_call": fl2 / (ms2 * 1e-3) / 1e12,
                                      "frac_of_nominal_fp8": fl2 / (ms2 * 1e-3) / 4.5e15,
                                      "frac_of_measured_fp8": fl2 / (ms2 * 1e-3) / (peak8 * 1e12),
+                                     "roofline": {"kernel": "gemm_tc_kernel<0> (gate/up + SwiGLU + requant)", "bound": "tensor",
+                                                  "achieved": 2.0 * 2 * cfg2.I * cfg2.H * (cfg2.T * (cfg2.k + cfg2.n_shared)) / (min(s["ms_gateup_sum"] for s in stats2) * 1e-3) / 1e12,
+                                                  "peak": peak8, "unit": "TFLOP/s", "traffic": NCU_TRAFFIC_BYTES["cfg2_resident"],
+                                                  "peak_source": "2 x bf16 measured (burst), fp8:bf16 nominal ratio",
+                                                  "sm_mhz_during_kernel": statistics.mean(s["sm_mhz_gateup"] for s in stats2)},
                                      "stage_ms": {k: statistics.mean(s[k] for s in stats2) for k in ("ms_route", "ms_experts", "ms_combine", "ms_gateup_sum", "ms_down_sum")}}
+            rr = extra["resident_32k"]["roofline"]
+            rr["frac"] = rr["achieved"] / rr["peak"]
             big.close()
         except Exception as ex:  # report, never hide
             extra["resident_32k"] = {"error": repr(ex)}

@@ -45,7 +45,6 @@ constexpr int kBoxRows = 64;  // rows per B TMA box
 constexpr int kEpiWarps = 8;
 constexpr int kThreads = (kEpiWarps + 4) * 32;  // three warpgroups: 2 x promotion, 1 x {producer, MMA, 2 idle}
 constexpr int kTmemCols = 512;
-constexpr int kScratchBytes = kEpiWarps * 32 * 32 * 4;  // per-warp 32 x 32 fp32 transpose tile (mode 1) / amax exchange (mode 0)
 constexpr int kMaxStages = 6;
 
 // kPair = false: one CTA per tile, A tile (16 KB) + whole B tile (32 KB) per stage, 4 stages.
@@ -53,12 +52,17 @@ constexpr int kMaxStages = 6;
 //                of the same expert) x N = 256; each CTA stages its own A tile and HALF of the B tile
 //                (16 KB + 16 KB per stage, 6 stages), which cuts the L2 -> SM operand traffic per MAC
 //                by a third (the 1-CTA kernel is L2-bandwidth bound, profiles/r1_gemm_baseline.md).
-template <bool kPair> struct Cfg {
-  static constexpr int kStages = kPair ? 6 : 4;
+template <int kMode, bool kPair> struct Cfg {
+  // The down kernel trades one pipeline stage for a four-deep Y staging ring per warp: its tiles are
+  // only 16 K blocks long, so the epilogue (128 KB of fp32 per tile) must not wait on TMA-store read-out.
+  static constexpr int kStages = kPair ? 6 : (kMode == 1 ? 3 : 4);
   static constexpr int kABytes = BM * BK;
   static constexpr int kBBytes = (kPair ? BN / 2 : BN) * BK;
   static constexpr int kStageBytes = kABytes + kBBytes;
+  static constexpr int kYRing = (kMode == 1 && !kPair) ? 4 : 2;              // 2 KB boxes per warp in flight
+  static constexpr int kScratchBytes = kEpiWarps * 2048 * kYRing;            // (mode 0: amax exchange only)
   static constexpr int kSmemBytes = kStages * kStageBytes + 1024 /*align*/ + 256 /*barriers*/ + kScratchBytes;
+  static_assert(kSmemBytes <= 232448, "shared memory budget");
 };
 
 // Barrier block behind the stage ring; the kernels address it through 32-bit shared addresses.
@@ -75,7 +79,12 @@ constexpr uint32_t kOffFull = 0, kOffEmpty = 8 * kMaxStages, kOffTmemFull = 16 *
 
 // silu(g) * u with the fast exponential and reciprocal (rel. error ~1e-6, three decades below the
 // e4m3 step that follows).
-__device__ __forceinline__ float silu_mul_fast(float g, float u) { return __fdividef(g, 1.0f + __expf(-g)) * u; }
+__device__ __forceinline__ float silu_mul_fast(float g, float u) {
+  float t, r;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(t) : "f"(g * -1.4426950408889634f));  // e^-g; overflow -> +inf -> r = 0
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(1.0f + t));
+  return g * r * u;
+}
 
 // Correctly rounded h / s from a correctly rounded reciprocal and one residual step (Markstein):
 // q0 = h * r, q = q0 + (h - q0 * s) * r.
@@ -93,8 +102,8 @@ template <int kMode, bool kPair>
 __global__ void __launch_bounds__(kThreads, 1)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__ CUtensorMap tm_b,
                const __grid_constant__ CUtensorMap tm_y, GemmArgs g) {
-  using C = Cfg<kPair>;
-  constexpr int kStages = C::kStages, kABytes = C::kABytes, kStageBytes = C::kStageBytes;
+  using C = Cfg<kMode, kPair>;
+  constexpr int kStages = C::kStages, kABytes = C::kABytes, kStageBytes = C::kStageBytes, kScratchBytes = C::kScratchBytes, kYRing = C::kYRing;
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   uint8_t* scratch = smem + kStages * kStageBytes;  // 1024-aligned: per-warp staging for the Y TMA stores / amax exchange
@@ -369,15 +378,19 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
         amax = fmaxf(amax, ex[(half ^ 1) * BM + r_in_tile]);
         const float s = (amax == 0.f) ? 1.0f : __fdiv_rn(amax, 448.0f);
         if (row_ok_cur) {
-          uint32_t pk[16];
-          if (s > 1e-30f) {
-            const float r = __frcp_rn(s);
+          // e4m3(h / s) with IEEE division semantics from one reciprocal + a residual step (div_by).  A
+          // denormal-range scale (never seen on real activations) is handled by scaling h and s by 2^64
+          // first, which is exact and leaves every quotient unchanged.
+          float sq = s;
+          if (s < 1e-30f) {
+            sq = s * 0x1p64f;
 #pragma unroll
-            for (int i = 0; i < 16; ++i) pk[i] = quant4_e4m3_r(acc[4 * i], acc[4 * i + 1], acc[4 * i + 2], acc[4 * i + 3], s, r);
-          } else {
-#pragma unroll
-            for (int i = 0; i < 16; ++i) pk[i] = quant4_e4m3(acc[4 * i], acc[4 * i + 1], acc[4 * i + 2], acc[4 * i + 3], s);
+            for (int i = 0; i < 64; ++i) acc[i] *= 0x1p64f;
           }
+          const float r = __frcp_rn(sq);
+          uint32_t pk[16];
+#pragma unroll
+          for (int i = 0; i < 16; ++i) pk[i] = quant4_e4m3_r(acc[4 * i], acc[4 * i + 1], acc[4 * i + 2], acc[4 * i + 3], sq, r);
           uint4* dst = reinterpret_cast<uint4*>(g.hq + row * g.I + nt * 128 + half * 64);
 #pragma unroll
           for (int i = 0; i < 4; ++i) dst[i] = make_uint4(pk[4 * i], pk[4 * i + 1], pk[4 * i + 2], pk[4 * i + 3]);
@@ -385,19 +398,18 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
         }
       } else {
         // Y tile (fp32, so that the layer's only bf16 rounding is the one in the combine): each warp owns
-        // 32 rows x 128 columns and streams them out as eight 32 x 16 boxes through a two-deep staging
-        // ring in shared memory (64-byte rows, 64B swizzle: conflict-free st.shared.v4) with TMA stores,
+        // 32 rows x 128 columns and streams them out as eight 32 x 16 boxes through a staging ring in shared memory (64-byte rows, 64B swizzle: conflict-free st.shared.v4) with TMA stores,
         // so the global writes drain asynchronously while the warp starts the next tile's K loop.
         // Rows past the expert's count are padding rows of the workspace; whole 32-row groups past it
         // are skipped.
         const int c0 = nt * BN + half * HN;
         if (c0 < g.H && q * 32 < nrows) {
-          const uint32_t stage_a = smem_a + kStages * kStageBytes + warp * 4096;  // 2 x 2 KB per warp
+          const uint32_t stage_a = smem_a + kStages * kStageBytes + warp * (2048 * kYRing);  // kYRing x 2 KB per warp
           const uint32_t sw = static_cast<uint32_t>((lane >> 1) & 3);
 #pragma unroll
           for (int c = 0; c < 8; ++c) {
-            const uint32_t dst = stage_a + (c & 1) * 2048;
-            if (lane == 0) ptx::bulk_wait_group_read<1>();  // the box that used this buffer two chunks ago has been read out
+            const uint32_t dst = stage_a + (c % kYRing) * 2048;
+            if (lane == 0) ptx::bulk_wait_group_read<kYRing - 1>();  // the box that used this buffer kYRing chunks ago has been read out
             __syncwarp();
 #pragma unroll
             for (int j = 0; j < 4; ++j) {

@@ -289,7 +289,7 @@ slp_status launch_experts(L* h, cudaStream_t s, int e_begin, int e_end, int T, i
       attr[0].val.clusterDim.z = 1;
       cudaLaunchConfig_t lc{};
       lc.blockDim = dim3(tc::kThreads);
-      lc.dynamicSmemBytes = tc::Cfg<true>::kSmemBytes;
+      lc.dynamicSmemBytes = tc::Cfg<0, true>::kSmemBytes;
       lc.stream = s;
       lc.attrs = attr;
       lc.numAttrs = 1;
@@ -297,13 +297,14 @@ slp_status launch_experts(L* h, cudaStream_t s, int e_begin, int e_end, int T, i
       CU_TRY(cudaLaunchKernelEx(&lc, tc::gemm_tc_kernel<0, true>, h->tm_xq, h->tm_wgu, h->tm_y, g0));
       if (ev) cudaEventRecord(ev[1], s);
       lc.gridDim = dim3(2 * std::max(1, std::min(n_cl, max_tiles * nt1)));
+      lc.dynamicSmemBytes = tc::Cfg<1, true>::kSmemBytes;
       CU_TRY(cudaLaunchKernelEx(&lc, tc::gemm_tc_kernel<1, true>, h->tm_hq, h->tm_wd, h->tm_y, g1));
     } else {
       const int grid0 = std::max(1, std::min(h->num_sms, max_tiles * nt0));
       const int grid1 = std::max(1, std::min(h->num_sms, max_tiles * nt1));
-      slp::tc::gemm_tc_kernel<0, false><<<grid0, slp::tc::kThreads, slp::tc::Cfg<false>::kSmemBytes, s>>>(h->tm_xq, h->tm_wgu, h->tm_y, g0);
+      slp::tc::gemm_tc_kernel<0, false><<<grid0, slp::tc::kThreads, slp::tc::Cfg<0, false>::kSmemBytes, s>>>(h->tm_xq, h->tm_wgu, h->tm_y, g0);
       if (ev) cudaEventRecord(ev[1], s);
-      slp::tc::gemm_tc_kernel<1, false><<<grid1, slp::tc::kThreads, slp::tc::Cfg<false>::kSmemBytes, s>>>(h->tm_hq, h->tm_wd, h->tm_y, g1);
+      slp::tc::gemm_tc_kernel<1, false><<<grid1, slp::tc::kThreads, slp::tc::Cfg<1, false>::kSmemBytes, s>>>(h->tm_hq, h->tm_wd, h->tm_y, g1);
     }
     if (ev) {
       cudaEventRecord(ev[2], s);
@@ -631,10 +632,10 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
   TRY_OR_BAIL(make_tmap_f32_store(&h->tm_y, h->d_y, H, rows));
   TRY_OR_BAIL(alloc_pool(h, n_stage, epl));
 
-  CU_OR_BAIL(cudaFuncSetAttribute(slp::tc::gemm_tc_kernel<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::tc::Cfg<true>::kSmemBytes));
-  CU_OR_BAIL(cudaFuncSetAttribute(slp::tc::gemm_tc_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::tc::Cfg<true>::kSmemBytes));
-  CU_OR_BAIL(cudaFuncSetAttribute(slp::tc::gemm_tc_kernel<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::tc::Cfg<false>::kSmemBytes));
-  CU_OR_BAIL(cudaFuncSetAttribute(slp::tc::gemm_tc_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::tc::Cfg<false>::kSmemBytes));
+  CU_OR_BAIL(cudaFuncSetAttribute(slp::tc::gemm_tc_kernel<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::tc::Cfg<0, true>::kSmemBytes));
+  CU_OR_BAIL(cudaFuncSetAttribute(slp::tc::gemm_tc_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::tc::Cfg<1, true>::kSmemBytes));
+  CU_OR_BAIL(cudaFuncSetAttribute(slp::tc::gemm_tc_kernel<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::tc::Cfg<0, false>::kSmemBytes));
+  CU_OR_BAIL(cudaFuncSetAttribute(slp::tc::gemm_tc_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::tc::Cfg<1, false>::kSmemBytes));
   CU_OR_BAIL(cudaDeviceSynchronize());
 #undef TRY_OR_BAIL
 #undef CU_OR_BAIL
