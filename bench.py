@@ -186,7 +186,7 @@ def main():
     # ------------------------------------------------------------------ our arm
     import __graft_entry__ as entry
     entry.build()
-    from paper_2606_10493_b200 import SlpMoeLayer, measure_h2d_gbs
+    from paper_2606_10493_b200 import SlpMoeLayer, measure_h2d_gbs, sharding
 
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU path)"
     torch.cuda.set_device(local_rank)
@@ -198,7 +198,7 @@ def main():
 
     t_gen = time.perf_counter()
     W = inputs.make_weights(cfg, device=dev, pin=True)
-    hidden = inputs.make_hidden(cfg, device=dev)
+    hidden = inputs.make_hidden(cfg, device=dev, first_chunk=sharding.weak_scaling_first_chunk(cfg.T, rank))  # each rank its own tokens
     t_gen = time.perf_counter() - t_gen
     layer = SlpMoeLayer(cfg, W, device=local_rank, staging_slots=args.staging_slots,
                         experts_per_launch=args.experts_per_launch, gemm_impl=args.gemm_impl)
@@ -230,11 +230,7 @@ def main():
 
     h2d_peak = measure_h2d_gbs(local_rank, 3 * cfg.I * cfg.H // 3, 1 << 30, 5) if mode == "streamed" else None
     ms, per_call, clocks = timed_steps(args.steps, ClockSampler(local_rank))
-    if world > 1:
-        t = torch.tensor([ms], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * cfg.T / (ms * 1e-3)
+    value, ms = sharding.whole_job_tokens_per_s(cfg.T, ms, device=dev)   # all ranks' tokens / slowest rank's device time
 
     # kernel-level numbers from the library's own CUDA events on the launching stream
     st = per_call[-1]
@@ -294,10 +290,7 @@ def main():
         for _ in range(n_e2e):
             layer.prefill_host(hin, hout)
         e2e_s = (time.perf_counter() - t0) / n_e2e
-        if world > 1:
-            t = torch.tensor([e2e_s], device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e2e_s = float(t.item())
+        e2e_s = sharding.max_over_ranks(e2e_s, device=dev)
         e2e = {"value": world * cfg.T / e2e_s, "unit": "tokens/s",
                "h2d_bytes_per_step": cfg.T * cfg.H * 2 + (st["bytes_copied"] if mode == "streamed" else 0),
                "d2h_bytes_per_step": cfg.T * cfg.H * 2}

@@ -1,34 +1,38 @@
 // kernels_gemm_tc.cuh — grouped FP8 GEMM on the 5th-gen tensor cores (a5, a6, a7, a8).
 //
-// One persistent CTA per SM walks a static round-robin list of (128-row tile, N tile) pairs over
-// the experts of the launch.  Per 128-deep K block the tensor core writes a fresh 128 x 256 fp32
-// partial into TMEM; the promotion warps pull it out with tcgen05.ld and add it into fp32 register
-// accumulators with one FMA per element, scaled by  xs[row, kb] * ws[n-block, kb]
-// ("FP8 GEMM with FP32 accumulation"; "accumulate all partial
-// dot-products first and apply the scale once per block").
+// One persistent CTA per SM walks a static round-robin list of (128-row tile, N tile) work items over
+// the experts of the launch (one 16-byte record per tile, written by permute_scan_kernel).  Per
+// 128-deep K block the tensor core writes a fresh 128 x 256 fp32 partial into one of two TMEM
+// buffers; the promotion warps pull it out with tcgen05.ld and add it into fp32 register accumulators
+// with one FMA per element (issued as FFMA2 pairs), scaled by  xs[row, kb] * ws[n-block, kb]
+// ("FP8 GEMM with FP32 accumulation"; "accumulate all partial dot-products
+// first and apply the scale once per block").
 //
-// The 256 accumulator columns of a K block are produced as two independent 128-column halves,
-// each with its own TMEM full/empty barrier pair and its own group of four promotion warps, and
-// TMEM holds two K blocks (4 half buffers).  Promotion of a half needs ~380 cycles of the ~512 a
-// K block takes on the tensor core, so the hand-off latencies only hide if a half can be refilled
-// three half-slots (768 cycles) after it was published (measured: profiles/r1_*).
-//
-//   warp 8      TMA producer: A tile (128 rows x 128 B) + four 64-row B boxes per K block into a
-//               4-stage 128B-swizzled smem ring (mbarrier full/empty)
-//   warp 9      MMA issuer: per K block and half, 4 x tcgen05.mma.kind::f8f6f4 (M128 N128 K32)
-//               into TMEM columns buf * 256 + half * 128; tcgen05.commit publishes the half and
-//               (after the second half) frees the smem stage
+//   warp 8      TMA producer (one elected thread): A tile (128 rows x 128 B) + 64-row B boxes per K
+//               block into a 128B-swizzled smem ring (mbarrier full / empty)
+//   warp 9      MMA issuer (one elected thread): per K block 4 x tcgen05.mma.kind::f8f6f4 (M128 N256
+//               K32) into TMEM buffer kb mod 2; tcgen05.commit publishes the buffer and frees the stage
 //   warps 10-11 idle (they only donate their registers, setmaxnreg)
-//   warps 0-7   promotion + epilogue: warp w owns TMEM lanes 32 * (w % 4).. (rows) of half w / 4;
-//               128 fp32 accumulators per thread
+//   warps 0-7   promotion + epilogue: warp w owns TMEM lanes 32 * (w % 4).. (rows) and the 128 columns
+//               of half w / 4; 128 fp32 accumulators per thread; the TMEM buffer is handed back as
+//               soon as the last tcgen05.ld has landed, before the last FMAs
+//
+// kPair (cfg.gemm_impl = 2): a cluster of two CTAs issues ONE cta_group::2 MMA with M = 256 (two
+//   128-row tiles of the same expert) x N = 256; each CTA stages its own A tile and half of the B tile
+//   (TMA loads of both CTAs complete on the leader's mbarrier, commits are multicast to both CTAs, the
+//   peer's promotion warps release TMEM on the leader's barrier).  It moves a third less operand data
+//   per MAC from L2 and through the shared-memory port; see DESIGN.md §6.1 for where each variant stands.
+//
+// All barrier / stage addresses are 32-bit shared-window addresses computed once (ptx::launder_u32):
+// re-deriving them from generic pointers cost ~100 of the ~285 instructions per warp per K block.
 //
 // kMode 0 (gate/up): B smem rows = [gate n0..+63 | up n0..+63 | gate n0+64..+127 | up n0+64..+127],
 //   so each half holds the gate and up columns of the same 64 intermediate channels; epilogue
 //   h = silu(g) * u, row amax over the 128 channels (two halves, exchanged through smem),
 //   s = amax / 448, e4m3(h / s) -> hq, hs  ("SiLU(.) (.)"; Q14).
-// kMode 1 (down):   B = down rows n0..n0+255; epilogue fp32 store of Y through a per-warp smem
-//   transpose so that every store instruction writes whole 128-byte lines (Y stays fp32 so that
-//   the only bf16 rounding of the layer is the final one in the combine).
+// kMode 1 (down):   B = down rows n0..n0+255; epilogue: the fp32 Y tile leaves through a per-warp
+//   staging ring in shared memory and TMA stores (Y stays fp32 so that the only bf16 rounding of the
+//   layer is the final one in the combine).
 #pragma once
 #include <cstdint>
 #include <cuda.h>

@@ -69,14 +69,15 @@ def _gen(cfg_seed, tensor, index, device):
     return g
 
 
-def make_hidden(cfg, device="cpu", T=None):
-    """bf16 N(0,1) hidden states [T, H], generated in independent 4096-row chunks."""
+def make_hidden(cfg, device="cpu", T=None, first_chunk=0):
+    """bf16 N(0,1) hidden states [T, H], generated in independent 4096-row chunks.  `first_chunk`
+    offsets the chunk index: rank r of a token-sharded run takes chunks [r * n, (r + 1) * n)."""
     T = cfg.T if T is None else T
     out = torch.empty((T, cfg.H), dtype=torch.bfloat16, device=device)
     for c in range((T + HIDDEN_CHUNK - 1) // HIDDEN_CHUNK):
         r0 = c * HIDDEN_CHUNK
         n = min(HIDDEN_CHUNK, T - r0)
-        x = torch.randn((HIDDEN_CHUNK, cfg.H), generator=_gen(cfg.seed, "hidden", c, device),
+        x = torch.randn((HIDDEN_CHUNK, cfg.H), generator=_gen(cfg.seed, "hidden", first_chunk + c, device),
                         device=device, dtype=torch.float32)
         out[r0:r0 + n] = x[:n].to(torch.bfloat16)
     return out
