@@ -328,36 +328,70 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
           ptx::mbar_wait_a(bar_a + kOffTmemFull + 8 * buf, (it >> 1) & 1, dead, g.err, 4);
           ptx::tc_fence_after();
           const uint32_t tb = tm_lane + buf * BN;
-          // 8 chunks of 16 columns, two register sets in flight; one FFMA2 per column pair
-          uint32_t v0[16], v1[16];
-          ptx::tmem_ld16(tb, v0);
-#pragma unroll
-          for (int c = 0; c < 8; c += 2) {
-            ptx::tmem_ld_wait16(v0);
-            ptx::tmem_ld16(tb + (c + 1) * 16, v1);
-            ptx::keep16(v0);  // v0 stays live across the issue of the next load: distinct registers
-            {
-              const uint64_t s2 = (c < 4) ? s20 : s21;
-#pragma unroll
-              for (int i = 0; i < 16; i += 2) ptx::fma2(acc2[c * 8 + i / 2], v0[i], v0[i + 1], s2);
+          if constexpr (kPair) {
+            // 8 chunks of 16 columns through four register sets: chunks 0-3 are loaded up front, chunk
+            // c + 4 is requested as soon as the FMAs of chunk c have consumed its set, so every
+            // tcgen05.ld of the K block has landed after half of the FMAs and the TMEM buffer goes back
+            // to the MMA issuer there (the hand-off round trip, not throughput, bounds the kernel).
+            uint32_t v[4][16];
+  #pragma unroll
+            for (int c = 0; c < 4; ++c) ptx::tmem_ld16(tb + c * 16, v[c]);
+            ptx::tmem_ld_wait16(v[0]);
+            ptx::keep16(v[1]); ptx::keep16(v[2]); ptx::keep16(v[3]);
+  #pragma unroll
+            for (int c = 0; c < 4; ++c) {
+              const uint64_t s2 = s20;  // chunks 0-3: gate columns (mode 0) / first weight-scale block
+  #pragma unroll
+              for (int i = 0; i < 16; i += 2) ptx::fma2(acc2[c * 8 + i / 2], v[c][i], v[c][i + 1], s2);
+              ptx::tmem_ld16(tb + (c + 4) * 16, v[c]);
             }
-            ptx::tmem_ld_wait16(v1);
-            if (c + 2 < 8) {
-              ptx::tmem_ld16(tb + (c + 2) * 16, v0);
-              ptx::keep16(v1);
-            } else {
-              // the whole partial is in registers: hand the TMEM buffer back before the last FMAs
-              ptx::tc_fence_before();
-              __syncwarp();
-              if (lane == 0) {
-                if (kPair && rank != 0) ptx::mbar_arrive_cluster(te_a + 8 * buf);  // remote: the leader's barrier
-                else ptx::mbar_arrive_a(bar_a + kOffTmemEmpty + 8 * buf);
+            ptx::tmem_ld_wait16(v[0]);
+            ptx::keep16(v[1]); ptx::keep16(v[2]); ptx::keep16(v[3]);
+            // the whole partial is in registers: hand the TMEM buffer back before the last FMAs
+            ptx::tc_fence_before();
+            __syncwarp();
+            if (lane == 0) {
+              if (kPair && rank != 0) ptx::mbar_arrive_cluster(te_a + 8 * buf);  // remote: the leader's barrier
+              else ptx::mbar_arrive_a(bar_a + kOffTmemEmpty + 8 * buf);
+            }
+  #pragma unroll
+            for (int c = 0; c < 4; ++c) {
+              const uint64_t s2 = s21;  // chunks 4-7: up columns (mode 0) / same block (mode 1: s21 == s20)
+  #pragma unroll
+              for (int i = 0; i < 16; i += 2) ptx::fma2(acc2[(c + 4) * 8 + i / 2], v[c][i], v[c][i + 1], s2);
+            }
+          } else {
+            // 8 chunks of 16 columns, two register sets in flight; one FFMA2 per column pair
+            uint32_t v0[16], v1[16];
+            ptx::tmem_ld16(tb, v0);
+  #pragma unroll
+            for (int c = 0; c < 8; c += 2) {
+              ptx::tmem_ld_wait16(v0);
+              ptx::tmem_ld16(tb + (c + 1) * 16, v1);
+              ptx::keep16(v0);  // v0 stays live across the issue of the next load: distinct registers
+              {
+                const uint64_t s2 = (c < 4) ? s20 : s21;
+  #pragma unroll
+                for (int i = 0; i < 16; i += 2) ptx::fma2(acc2[c * 8 + i / 2], v0[i], v0[i + 1], s2);
               }
-            }
-            {
-              const uint64_t s2 = (c + 1 < 4) ? s20 : s21;
-#pragma unroll
-              for (int i = 0; i < 16; i += 2) ptx::fma2(acc2[(c + 1) * 8 + i / 2], v1[i], v1[i + 1], s2);
+              ptx::tmem_ld_wait16(v1);
+              if (c + 2 < 8) {
+                ptx::tmem_ld16(tb + (c + 2) * 16, v0);
+                ptx::keep16(v1);
+              } else {
+                // the whole partial is in registers: hand the TMEM buffer back before the last FMAs
+                ptx::tc_fence_before();
+                __syncwarp();
+                if (lane == 0) {
+                  if (kPair && rank != 0) ptx::mbar_arrive_cluster(te_a + 8 * buf);  // remote: the leader's barrier
+                  else ptx::mbar_arrive_a(bar_a + kOffTmemEmpty + 8 * buf);
+                }
+              }
+              {
+                const uint64_t s2 = (c + 1 < 4) ? s20 : s21;
+  #pragma unroll
+                for (int i = 0; i < 16; i += 2) ptx::fma2(acc2[(c + 1) * 8 + i / 2], v1[i], v1[i + 1], s2);
+              }
             }
           }
           ++it;
