@@ -114,14 +114,32 @@ def test_layer_parity_simt(name, mode):
 @pytest.mark.parametrize("name", list(CASES))
 @pytest.mark.parametrize("mode", ["resident", "streamed"])
 def test_layer_parity_tcgen05(name, mode):
-    """gemm_impl 0: the product path, cta_group::2 MMA over a cluster of two CTAs (pairs of 128-row tiles)."""
+    """gemm_impl 0: the product path (tcgen05 / TMEM / TMA, one CTA per 128 x 256 tile)."""
     check(name, mode, gemm_impl=0)
 
 
 @pytest.mark.parametrize("name", list(CASES))
-def test_layer_parity_tcgen05_single_cta(name):
-    """gemm_impl 2: the one-CTA-per-tile variant of the same kernel (kept for triage)."""
+def test_layer_parity_tcgen05_cta_pair(name):
+    """gemm_impl 2: the cta_group::2 variant (clusters of two CTAs, pairs of 128-row tiles, dummy
+    tile for experts with an odd tile count)."""
     check(name, "resident", gemm_impl=2)
+
+
+@pytest.mark.parametrize("T", [1, 127, 128, 129, 257])
+@pytest.mark.parametrize("gemm_impl", [0, 2])
+def test_ragged_token_counts(T, gemm_impl):
+    """Edge sizes: a single token, one row short of / exactly / one row past a 128-row tile."""
+    cfg, W, hidden, _ = problem("mini_dsv3")
+    sub = cfg.with_tokens(T)
+    x = hidden[:T].contiguous()
+    ref = moe_layer(inputs.hidden_as_bits(x), inputs.weights_as_numpy(W), top_k=cfg.k, n_group=cfg.G,
+                    topk_group=cfg.Gk, scoring=cfg.scoring, norm_topk=cfg.norm_topk, routed_scale=cfg.routed_scale)
+    for mode in ("resident", "streamed"):
+        out, idx, w, counts, *_ = run_gpu(sub, W, x, mode, gemm_impl=gemm_impl)
+        r = compare_routing(idx, w, ref["route"])
+        o = compare_output(out, ref["out_f64"], r["members_equal"])
+        assert r["passed"] and o["passed"], (T, mode, r, o)
+        assert counts.sum() == T * cfg.k
 
 
 @pytest.mark.parametrize("name", list(CASES))
