@@ -90,6 +90,13 @@ __device__ __forceinline__ float silu_mul_fast(float g, float u) {
   return g * r * u;
 }
 
+// p ? a : b as one SELP (keeps the scale bookkeeping of the K loop free of branches and copies).
+__device__ __forceinline__ float sel_f32(bool p, float a, float b) {
+  float r;
+  asm("{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %3, 0;\n\tselp.f32 %0, %1, %2, q;\n\t}" : "=f"(r) : "f"(a), "f"(b), "r"(static_cast<int>(p)));
+  return r;
+}
+
 // Correctly rounded h / s from a correctly rounded reciprocal and one residual step (Markstein):
 // q0 = h * r, q = q0 + (h - q0 * s) * r.
 __device__ __forceinline__ float div_by(float h, float s, float r) {
@@ -308,19 +315,26 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
 #pragma unroll 1
       for (int kb = 0; kb < num_kb; ++kb) {
         {
-          if ((kb & 3) == 0) {
-            xs_cur = xs_nxt;
+          // Branch-free scale bookkeeping (selp): a branchy version cost ~40 MOV / BRA per K block in
+          // an issue-bound loop.  Every 4th K block the row's next four activation scales (one 16-byte
+          // load issued a group ahead) become current; every 32nd the lane-held weight scales rotate.
+          const int j = kb & 3;
+          const bool g4 = j == 0, g32 = (kb & 31) == 0;
+          xs_cur.x = sel_f32(g4, xs_nxt.x, xs_cur.x);
+          xs_cur.y = sel_f32(g4, xs_nxt.y, xs_cur.y);
+          xs_cur.z = sel_f32(g4, xs_nxt.z, xs_cur.z);
+          xs_cur.w = sel_f32(g4, xs_nxt.w, xs_cur.w);
+          w0_cur = sel_f32(g32, w0_nxt, w0_cur);
+          w1_cur = sel_f32(g32, w1_nxt, w1_cur);
+          if (g4) {
             if (kb + 4 < num_kb && row_ok) xs_nxt = *reinterpret_cast<const float4*>(as_ptr + kb + 4);
-            if ((kb & 31) == 0) {
-              w0_cur = w0_nxt;
-              w1_cur = w1_nxt;
+            if (g32) {
               const int kn = kb + 32 + lane;
               w0_nxt = kn < num_kb ? ws0[kn] : 0.f;
               w1_nxt = (kMode == 0 && kn < num_kb) ? ws1[kn] : 0.f;
             }
           }
-          const int j = kb & 3;
-          const float sa = j == 0 ? xs_cur.x : j == 1 ? xs_cur.y : j == 2 ? xs_cur.z : xs_cur.w;
+          const float sa = sel_f32((j & 2) != 0, sel_f32((j & 1) != 0, xs_cur.w, xs_cur.z), sel_f32((j & 1) != 0, xs_cur.y, xs_cur.x));
           const float sc0 = sa * __shfl_sync(0xFFFFFFFFu, w0_cur, kb & 31);
           const float sc1 = kMode == 0 ? sa * __shfl_sync(0xFFFFFFFFu, w1_cur, kb & 31) : sc0;
           const uint64_t s20 = ptx::pack2(sc0, sc0), s21 = ptx::pack2(sc1, sc1);
@@ -366,18 +380,16 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
             ptx::tmem_ld16(tb, v0);
   #pragma unroll
             for (int c = 0; c < 8; c += 2) {
-              ptx::tmem_ld_wait16(v0);
+              ptx::tmem_ld_wait();
               ptx::tmem_ld16(tb + (c + 1) * 16, v1);
-              ptx::keep16(v0);  // v0 stays live across the issue of the next load: distinct registers
               {
                 const uint64_t s2 = (c < 4) ? s20 : s21;
   #pragma unroll
                 for (int i = 0; i < 16; i += 2) ptx::fma2(acc2[c * 8 + i / 2], v0[i], v0[i + 1], s2);
               }
-              ptx::tmem_ld_wait16(v1);
+              ptx::tmem_ld_wait();
               if (c + 2 < 8) {
                 ptx::tmem_ld16(tb + (c + 2) * 16, v0);
-                ptx::keep16(v1);
               } else {
                 // the whole partial is in registers: hand the TMEM buffer back before the last FMAs
                 ptx::tc_fence_before();
