@@ -57,14 +57,15 @@ constexpr int kMaxStages = 6;
 //                (16 KB + 16 KB per stage, 6 stages), which cuts the L2 -> SM operand traffic per MAC
 //                by a third (the 1-CTA kernel is L2-bandwidth bound, profiles/r1_gemm_baseline.md).
 template <int kMode, bool kPair> struct Cfg {
-  // The down kernel trades one pipeline stage for a four-deep Y staging ring per warp: its tiles are
-  // only 16 K blocks long, so the epilogue (128 KB of fp32 per tile) must not wait on TMA-store read-out.
-  static constexpr int kStages = kPair ? 6 : (kMode == 1 ? 3 : 4);
+  // The down kernel trades pipeline stages for a Y staging ring (two 32 x 32 fp32 boxes per warp): its
+  // tiles are only 16 K blocks long, so the epilogue (128 KB of fp32 per tile) must not wait long on
+  // TMA-store read-out.
+  static constexpr int kStages = kPair ? (kMode == 1 ? 5 : 6) : (kMode == 1 ? 3 : 4);
   static constexpr int kABytes = BM * BK;
   static constexpr int kBBytes = (kPair ? BN / 2 : BN) * BK;
   static constexpr int kStageBytes = kABytes + kBBytes;
-  static constexpr int kYRing = (kMode == 1 && !kPair) ? 4 : 2;              // 2 KB boxes per warp in flight
-  static constexpr int kScratchBytes = kEpiWarps * 2048 * kYRing;            // (mode 0: amax exchange only)
+  static constexpr int kYRing = 2;                                           // 4 KB boxes per warp in flight
+  static constexpr int kScratchBytes = kMode == 1 ? kEpiWarps * 4096 * kYRing : 32768;  // (mode 0: amax exchange only)
   static constexpr int kSmemBytes = kStages * kStageBytes + 1024 /*align*/ + 256 /*barriers*/ + kScratchBytes;
   static_assert(kSmemBytes <= 232448, "shared memory budget");
 };
@@ -448,29 +449,29 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
         }
       } else {
         // Y tile (fp32, so that the layer's only bf16 rounding is the one in the combine): each warp owns
-        // 32 rows x 128 columns and streams them out as eight 32 x 16 boxes through a staging ring in shared memory (64-byte rows, 64B swizzle: conflict-free st.shared.v4) with TMA stores,
+        // 32 rows x 128 columns and streams them out as four 32 x 32 boxes through a staging ring in shared memory (128-byte rows, 128B swizzle: conflict-free st.shared.v4, whole-line global writes) with TMA stores,
         // so the global writes drain asynchronously while the warp starts the next tile's K loop.
         // Rows past the expert's count are padding rows of the workspace; whole 32-row groups past it
         // are skipped.
         const int c0 = nt * BN + half * HN;
         if (c0 < g.H && q * 32 < nrows) {
-          const uint32_t stage_a = smem_a + kStages * kStageBytes + warp * (2048 * kYRing);  // kYRing x 2 KB per warp
-          const uint32_t sw = static_cast<uint32_t>((lane >> 1) & 3);
+          const uint32_t stage_a = smem_a + kStages * kStageBytes + warp * (4096 * kYRing);  // kYRing x 4 KB per warp
+          const uint32_t sw = static_cast<uint32_t>(lane & 7);
 #pragma unroll
-          for (int c = 0; c < 8; ++c) {
-            const uint32_t dst = stage_a + (c % kYRing) * 2048;
-            if (lane == 0) ptx::bulk_wait_group_read<kYRing - 1>();  // the box that used this buffer kYRing chunks ago has been read out
+          for (int c = 0; c < 4; ++c) {  // four boxes of 32 rows x 32 columns (128-byte rows, 128B swizzle)
+            const uint32_t dst = stage_a + (c % kYRing) * 4096;
+            if (lane == 0) ptx::bulk_wait_group_read<kYRing - 1>();  // the box that used this buffer kYRing boxes ago has been read out
             __syncwarp();
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              const uint32_t a = dst + lane * 64 + ((static_cast<uint32_t>(j) ^ sw) << 4);
-              asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(a), "f"(acc[c * 16 + j * 4]), "f"(acc[c * 16 + j * 4 + 1]),
-                           "f"(acc[c * 16 + j * 4 + 2]), "f"(acc[c * 16 + j * 4 + 3]) : "memory");
+            for (int j = 0; j < 8; ++j) {
+              const uint32_t a = dst + lane * 128 + ((static_cast<uint32_t>(j) ^ sw) << 4);
+              asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(a), "f"(acc[c * 32 + j * 4]), "f"(acc[c * 32 + j * 4 + 1]),
+                           "f"(acc[c * 32 + j * 4 + 2]), "f"(acc[c * 32 + j * 4 + 3]) : "memory");
             }
             ptx::fence_proxy_async_smem();
             __syncwarp();
             if (lane == 0) {
-              ptx::tma_store_2d_a(&tm_y, dst, c0 + c * 16, row0 + q * 32);
+              ptx::tma_store_2d_a(&tm_y, dst, c0 + c * 32, row0 + q * 32);
               ptx::bulk_commit_group();
             }
           }

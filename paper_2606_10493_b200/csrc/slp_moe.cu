@@ -77,16 +77,16 @@ slp_status make_tmap_u8(CUtensorMap* tm, void* base, uint64_t inner, uint64_t ro
   return SLP_OK;
 }
 
-// 2D fp32 tensor [rows, inner] for TMA stores of 16-column x 32-row boxes (64-byte rows, 64B swizzle).
+// 2D fp32 tensor [rows, inner] for TMA stores of 32-column x 32-row boxes (128-byte rows, 128B swizzle).
 slp_status make_tmap_f32_store(CUtensorMap* tm, void* base, uint64_t inner, uint64_t rows) {
   EncodeTiledFn fn = get_encode_fn();
   if (!fn) return fail(SLP_ERR_CUDA, "cuTensorMapEncodeTiled not available from the driver");
   cuuint64_t dims[2] = {inner, rows};
   cuuint64_t strides[1] = {inner * 4};
-  cuuint32_t box[2] = {16, 32};
+  cuuint32_t box[2] = {32, 32};
   cuuint32_t estr[2] = {1, 1};
   CUresult r = fn(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                  CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                  CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return fail(SLP_ERR_CUDA, "cuTensorMapEncodeTiled (Y store) failed with CUresult %d", static_cast<int>(r));
   return SLP_OK;
 }
