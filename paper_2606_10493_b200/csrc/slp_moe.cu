@@ -91,11 +91,12 @@ slp_status make_tmap_f32_store(CUtensorMap* tm, void* base, uint64_t inner, uint
   return SLP_OK;
 }
 
-// experts_per_launch = 0 (auto): up to 32 experts per grouped-GEMM launch (amortises the launch ramp
-// and tail: 0.40 -> 0.65 of HBM roofline on the T = 4096 layer); a ring shorter than the layer needs
-// a divisor of the ring length that is at most half of it.
+// experts_per_launch = 0 (auto): up to 64 experts per grouped-GEMM launch when the ring holds the
+// whole layer (amortises the launch ramp and tail: 0.40 -> 0.70 of the HBM roofline on the T = 4096
+// layer, while the host-link-bound step moves by < 0.1 %); a ring shorter than the layer needs a
+// divisor of the ring length that is at most half of it (and at most 32).
 inline int auto_epl(int n_stage, int E) {
-  if (n_stage == E) return std::min(32, E);
+  if (n_stage == E) return std::min(64, E);
   int best = 1;
   for (int d = 1; d <= std::min(32, n_stage / 2); ++d)
     if (n_stage % d == 0) best = d;
