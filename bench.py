@@ -38,7 +38,7 @@ WORKLOADS = {
 METRIC = "prefill tok/s per MoE layer (host-streamed FP8); resident FP8 TFLOP/s vs peak"
 # dram__bytes_read.sum + dram__bytes_write.sum of one gemm_tc_kernel<0> launch, from the committed ncu
 # --set full captures (profiles/r1_layer_ncu.md, profiles/r1_streamed_gemm_ncu.md); None = not captured.
-NCU_TRAFFIC_BYTES = {"cfg2_resident": 27.91e9, "cfg1_streamed": 1.028e9}
+NCU_TRAFFIC_BYTES = {"cfg2_resident": 10.65e9, "cfg1_streamed": 2.143e9}
 
 
 def load_peaks():

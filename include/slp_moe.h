@@ -78,11 +78,13 @@ typedef struct {
                                  prefill).  0: paper-faithful fixed order, every expert copied. */
   int32_t require_pinned;     /* 1: create fails with SLP_ERR_NOT_PINNED if a weight buffer is
                                  pageable.  0: create pins it with cudaHostRegister. */
-  int32_t gemm_impl;          /* 0: tcgen05/TMEM/TMA grouped GEMM, cta_group::2 MMA over clusters of two
-                                    CTAs (the product path).
-                                 1: plain CUDA-core grouped GEMM kept for bring-up and for
-                                    triaging the tensor-core kernels; same kernels around it.
-                                 2: the one-CTA-per-tile variant of the tcgen05 kernel (triage). */
+  int32_t gemm_impl;          /* 0: tcgen05/TMEM/TMA grouped GEMM, one CTA per 128 x 256 tile, tiles handed out
+                                    through a global counter (the product path).
+                                 1: plain CUDA-core grouped GEMM kept for bring-up and for triaging the
+                                    tensor-core kernels; same kernels around it.
+                                 2: the cta_group::2 variant of the tcgen05 kernel (clusters of two CTAs).
+                                 3: as 0 with a static round-robin tile order (reads the operands from DRAM
+                                    ~2.7 times instead of once; kept for A/B). */
   int32_t router_impl;        /* 0: router logits on the tensor cores (bf16 hi+lo split of the fp32
                                  router weights, fp32 accumulate).  1: plain fp32 FMA kernel
                                  (bring-up / triage). */

@@ -38,6 +38,7 @@ struct GemmArgs {
   int hs_stride;
   float* y;                    // [rows, H] fp32
   int* err;
+  int* sched;                  // [2] work-item counters of the gate/up and down launches (zeroed before each launch pair)
   unsigned long long* clk;     // [4] {SM cycles, ns} of CTA 0 summed over gate/up launches, then over down launches
 };
 

@@ -1,7 +1,9 @@
 // kernels_gemm_tc.cuh — grouped FP8 GEMM on the 5th-gen tensor cores (a5, a6, a7, a8).
 //
-// One persistent CTA per SM walks a static round-robin list of (128-row tile, N tile) work items over
-// the experts of the launch (one 16-byte record per tile, written by permute_scan_kernel).  Per
+// One persistent CTA per SM works through the (128-row tile, N tile) work items of the experts of the
+// launch (one 16-byte record per tile, written by permute_scan_kernel); an otherwise idle warp takes the
+// items from a global counter, so all CTAs stay within ~gridDim consecutive items and share operands
+// through L2 (cfg.gemm_impl = 3: static round-robin instead).  Per
 // 128-deep K block the tensor core writes a fresh 128 x 256 fp32 partial into one of two TMEM
 // buffers; the promotion warps pull it out with tcgen05.ld and add it into fp32 register accumulators
 // with one FMA per element (issued as FFMA2 pairs), scaled by  xs[row, kb] * ws[n-block, kb]
@@ -12,7 +14,9 @@
 //               block into a 128B-swizzled smem ring (mbarrier full / empty)
 //   warp 9      MMA issuer (one elected thread): per K block 4 x tcgen05.mma.kind::f8f6f4 (M128 N256
 //               K32) into TMEM buffer kb mod 2; tcgen05.commit publishes the buffer and frees the stage
-//   warps 10-11 idle (they only donate their registers, setmaxnreg)
+//   warp 10     work scheduler (one elected thread): atomicAdd on the launch's counter -> 4-deep smem ring
+//               read by the producer, the MMA issuer and the promotion warps
+//   warp 11     idle (warps 8-11 donate most of their registers to the promotion warps, setmaxnreg)
 //   warps 0-7   promotion + epilogue: warp w owns TMEM lanes 32 * (w % 4).. (rows) and the 128 columns
 //               of half w / 4; 128 fp32 accumulators per thread; the TMEM buffer is handed back as
 //               soon as the last tcgen05.ld has landed, before the last FMAs
@@ -50,6 +54,7 @@ constexpr int kEpiWarps = 8;
 constexpr int kThreads = (kEpiWarps + 4) * 32;  // three warpgroups: 2 x promotion, 1 x {producer, MMA, 2 idle}
 constexpr int kTmemCols = 512;
 constexpr int kMaxStages = 6;
+constexpr int kSchedDepth = 4;  // work items the scheduler warp may run ahead of the roles
 
 // kPair = false: one CTA per tile, A tile (16 KB) + whole B tile (32 KB) per stage, 4 stages.
 // kPair = true:  a cluster of two CTAs issues one cta_group::2 MMA with M = 256 (two 128-row tiles
@@ -76,11 +81,15 @@ struct Shared {
   uint64_t empty[kMaxStages];  // MMA -> TMA: stage consumed (pair: multicast commit to both CTAs)
   uint64_t tmem_full[2];       // MMA -> promotion: K block partial complete in TMEM buffer b
   uint64_t tmem_empty[2];      // promotion -> MMA: buffer b read out (pair: 2 x kEpiWarps arrivals at the leader)
+  uint64_t sched_full[kSchedDepth];   // scheduler -> roles: work item published
+  uint64_t sched_empty[kSchedDepth];  // roles -> scheduler: slot read by producer, MMA issuer and the promotion warps
+  int32_t sched_w[kSchedDepth];       // work item of each slot (-1 = no more work)
   uint32_t tmem_base;
   int dead;
 };
 static_assert(sizeof(Shared) <= 256, "barrier block");
 constexpr uint32_t kOffFull = 0, kOffEmpty = 8 * kMaxStages, kOffTmemFull = 16 * kMaxStages, kOffTmemEmpty = 16 * kMaxStages + 16;
+constexpr uint32_t kOffSchedFull = kOffTmemEmpty + 16, kOffSchedEmpty = kOffSchedFull + 8 * kSchedDepth;
 
 // silu(g) * u with the fast exponential and reciprocal (rel. error ~1e-6, three decades below the
 // e4m3 step that follows).
@@ -110,7 +119,7 @@ __device__ __forceinline__ uint32_t quant4_e4m3_r(float a, float b, float c, flo
   return static_cast<uint32_t>(lo) | (static_cast<uint32_t>(hi) << 16);
 }
 
-template <int kMode, bool kPair>
+template <int kMode, bool kPair, bool kDyn = false>
 __global__ void __launch_bounds__(kThreads, 1)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__ CUtensorMap tm_b,
                const __grid_constant__ CUtensorMap tm_y, GemmArgs g) {
@@ -146,6 +155,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
   if (threadIdx.x == 0) {
     for (int i = 0; i < kStages; ++i) { ptx::mbar_init(&sh->full[i], 1); ptx::mbar_init(&sh->empty[i], 1); }
     for (int i = 0; i < 2; ++i) { ptx::mbar_init(&sh->tmem_full[i], 1); ptx::mbar_init(&sh->tmem_empty[i], kPair ? 2 * kEpiWarps : kEpiWarps); }
+    for (int i = 0; i < kSchedDepth; ++i) { ptx::mbar_init(&sh->sched_full[i], 1); ptx::mbar_init(&sh->sched_empty[i], 2 + kEpiWarps); }
     sh->dead = 0;
     ptx::fence_mbar_init();
   }
@@ -186,6 +196,27 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
     return t;
   };
 
+  // Next work item of this CTA after `w` (its i-th), or -1.  Static order: w + gridDim.  kDyn (one-CTA
+  // kernel, the default; cfg.gemm_impl = 3 selects the static order): items come from a global counter through a small shared-memory ring fed by an idle warp, so
+  // all CTAs stay inside a window of ~gridDim consecutive items and the B tiles they share stay in L2
+  // (profiles/r1_sched_ab.md).  Which CTA computes a tile does not change its result.
+  auto next_item = [&](int w, int i, bool whole_warp) -> int {
+    if constexpr (kPair || !kDyn) {
+      w += w_step;
+    } else {
+      const uint32_t slot = static_cast<uint32_t>(i) % kSchedDepth;
+      ptx::mbar_wait_a(bar_a + kOffSchedFull + 8 * slot, (static_cast<uint32_t>(i) / kSchedDepth) & 1, dead, g.err, 5);
+      w = sh->sched_w[slot];  // plain load from a warp-uniform address (the wait above is a compiler barrier)
+      if (whole_warp) {
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive_a(bar_a + kOffSchedEmpty + 8 * slot);
+      } else {
+        ptx::mbar_arrive_a(bar_a + kOffSchedEmpty + 8 * slot);
+      }
+    }
+    return w < total ? w : -1;
+  };
+
   // Registers: 168 per thread at launch (384 threads); the producer / MMA warpgroup gives most of
   // its share to the two promotion warpgroups, which hold 128 accumulators + two loads in flight.
   if (warp >= kEpiWarps) {
@@ -196,9 +227,11 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
       int stage = 0;
       uint32_t phase = 0;
       Tile nx = fetch(min(w_first, max(total - 1, 0)));
-      for (int w = w_first; w < total; w += w_step) {
+      int w = w_first < total ? w_first : -1;
+      for (int i = 0; w >= 0; ++i) {
         const Tile cur = nx;
-        if (w + w_step < total) nx = fetch(w + w_step);  // next tile's record is in flight during this tile's loads
+        w = next_item(w, i, false);
+        if (w >= 0) nx = fetch(w);  // next tile's record is in flight during this tile's loads
         const int e = cur.e, nt = cur.nt, row0 = cur.row0;
         const int slot = slot_of(g, e);
         constexpr int kBoxes = kPair ? 2 : 4;
@@ -232,6 +265,18 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
         }
       }
     }
+   } else if (warp == kEpiWarps + 2) {
+    // ===================== work scheduler (kDyn; one elected thread) =====================
+    if (!kPair && kDyn && ptx::elect_one()) {
+      for (int i = 0;; ++i) {  // slot i holds the item that FOLLOWS this CTA's i-th item (the first is blockIdx)
+        const uint32_t slot = static_cast<uint32_t>(i) % kSchedDepth;
+        ptx::mbar_wait_a(bar_a + kOffSchedEmpty + 8 * slot, ((static_cast<uint32_t>(i) / kSchedDepth) & 1) ^ 1, dead, g.err, 6);
+        const int w = static_cast<int>(gridDim.x) + atomicAdd(g.sched + kMode, 1);
+        sh->sched_w[slot] = w;
+        ptx::mbar_arrive_a(bar_a + kOffSchedFull + 8 * slot);  // release: the store above is visible to the waiters
+        if (w >= total) break;
+      }
+    }
    } else if (warp == kEpiWarps + 1) {
     // ===================== MMA issuer (one elected thread; pair: leader CTA only) =====================
     if (rank == 0 && ptx::elect_one()) {
@@ -240,7 +285,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
       int stage = 0;
       uint32_t phase = 0;
       uint32_t it = 0;  // running K-block counter: TMEM buffer = it & 1
-      for (int w = w_first; w < total; w += w_step) {
+      int w = w_first < total ? w_first : -1;
+      for (int i = 0; w >= 0; w = next_item(w, i, false), ++i) {
         for (int kb = 0; kb < num_kb; ++kb, ++it) {
           const uint32_t buf = it & 1, tph = ((it >> 1) & 1) ^ 1;
           ptx::mbar_wait_a(bar_a + kOffFull + 8 * stage, phase, dead, g.err, 3);    // operands landed (usually long ago)
@@ -300,10 +346,12 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
     };
     Tile nx = fetch(min(w_first, max(total - 1, 0)));
     if (w_first < total) open_tile(nx);
-    for (int w = w_first; w < total; w += w_step, tile_parity ^= 1) {
+    int w = w_first < total ? w_first : -1;
+    for (int i = 0; w >= 0; ++i, tile_parity ^= 1) {
       const Tile cur = nx;
-      const bool has_next = w + w_step < total;
-      if (has_next) nx = fetch(w + w_step);  // record in flight during the K loop
+      w = next_item(w, i, true);
+      const bool has_next = w >= 0;
+      if (has_next) nx = fetch(w);  // record in flight during the K loop
       const int nt = cur.nt, row0 = cur.row0, nrows = cur.nrows;
       const size_t row = static_cast<size_t>(row0 + r_in_tile);
       const bool row_ok_cur = row_ok;

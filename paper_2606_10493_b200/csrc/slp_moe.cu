@@ -136,6 +136,7 @@ struct slp_moe_layer {
   float* d_y = nullptr;
   int* d_err = nullptr;
   unsigned long long* d_clk = nullptr;
+  int* d_sched = nullptr;
   void *d_e2e_in = nullptr, *d_e2e_out = nullptr;
   int32_t* h_counts = nullptr;  // pinned
   int* h_err = nullptr;         // pinned
@@ -263,6 +264,7 @@ slp::GemmArgs gemm_args(L* h, int mode, int e_begin, int e_end, int T) {
   g.y = h->d_y;
   g.err = h->d_err;
   g.clk = h->d_clk;
+  g.sched = h->d_sched;
   return g;
 }
 
@@ -278,6 +280,7 @@ slp_status launch_experts(L* h, cudaStream_t s, int e_begin, int e_end, int T, i
     slp::GemmArgs g0 = gemm_args(h, 0, e_begin, e_end, T), g1 = gemm_args(h, 1, e_begin, e_end, T);
     const int nt0 = h->I / 128, nt1 = (h->H + 255) / 256;
     cudaEvent_t* ev = (h->ev_k_used + 3 <= static_cast<int>(h->ev_k.size())) ? &h->ev_k[h->ev_k_used] : nullptr;
+    if (h->cfg.gemm_impl == 0) CU_TRY(cudaMemsetAsync(h->d_sched, 0, 2 * sizeof(int), s));  // work-item counters of the two launches below
     if (ev) cudaEventRecord(ev[0], s);
     if (h->cfg.gemm_impl == 2) {
       // CTA-pair kernel: clusters of two CTAs, one per SM; a work item is a pair of 128-row tiles
@@ -303,9 +306,16 @@ slp_status launch_experts(L* h, cudaStream_t s, int e_begin, int e_end, int T, i
     } else {
       const int grid0 = std::max(1, std::min(h->num_sms, max_tiles * nt0));
       const int grid1 = std::max(1, std::min(h->num_sms, max_tiles * nt1));
-      slp::tc::gemm_tc_kernel<0, false><<<grid0, slp::tc::kThreads, slp::tc::Cfg<0, false>::kSmemBytes, s>>>(h->tm_xq, h->tm_wgu, h->tm_y, g0);
-      if (ev) cudaEventRecord(ev[1], s);
-      slp::tc::gemm_tc_kernel<1, false><<<grid1, slp::tc::kThreads, slp::tc::Cfg<1, false>::kSmemBytes, s>>>(h->tm_hq, h->tm_wd, h->tm_y, g1);
+      namespace tc = slp::tc;
+      if (h->cfg.gemm_impl == 0) {  // dynamic tile distribution (the product path); 3 = static round-robin
+        tc::gemm_tc_kernel<0, false, true><<<grid0, tc::kThreads, tc::Cfg<0, false>::kSmemBytes, s>>>(h->tm_xq, h->tm_wgu, h->tm_y, g0);
+        if (ev) cudaEventRecord(ev[1], s);
+        tc::gemm_tc_kernel<1, false, true><<<grid1, tc::kThreads, tc::Cfg<1, false>::kSmemBytes, s>>>(h->tm_hq, h->tm_wd, h->tm_y, g1);
+      } else {
+        tc::gemm_tc_kernel<0, false><<<grid0, tc::kThreads, tc::Cfg<0, false>::kSmemBytes, s>>>(h->tm_xq, h->tm_wgu, h->tm_y, g0);
+        if (ev) cudaEventRecord(ev[1], s);
+        tc::gemm_tc_kernel<1, false><<<grid1, tc::kThreads, tc::Cfg<1, false>::kSmemBytes, s>>>(h->tm_hq, h->tm_wd, h->tm_y, g1);
+      }
     }
     if (ev) {
       cudaEventRecord(ev[2], s);
@@ -486,7 +496,7 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
     return fail(SLP_ERR_UNSUPPORTED_SHAPE, "n_shared must be 0 or 1 with shared_intermediate == moe_intermediate");
   if (cfg->scoring != SLP_SCORE_SIGMOID_BIAS && cfg->scoring != SLP_SCORE_SOFTMAX) return fail(SLP_ERR_INVALID_ARG, "unknown scoring %d", cfg->scoring);
   if (cfg->max_tokens <= 0) return fail(SLP_ERR_INVALID_ARG, "max_tokens must be positive");
-  if (cfg->gemm_impl < 0 || cfg->gemm_impl > 2) return fail(SLP_ERR_INVALID_ARG, "gemm_impl must be 0, 1 or 2");
+  if (cfg->gemm_impl < 0 || cfg->gemm_impl > 3) return fail(SLP_ERR_INVALID_ARG, "gemm_impl must be 0, 1, 2 or 3");
   if (cfg->router_impl != 0 && cfg->router_impl != 1) return fail(SLP_ERR_INVALID_ARG, "router_impl must be 0 or 1");
   int n_stage = cfg->staging_slots == 0 ? E : cfg->staging_slots;
   if (n_stage < 2 && E >= 2) return fail(SLP_ERR_INVALID_ARG, "staging_slots must be 0 or 2..n_experts");
@@ -619,6 +629,7 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
   CU_OR_BAIL(cudaMalloc(&h->d_hs, rows * h->hs_stride * sizeof(float)));
   CU_OR_BAIL(cudaMalloc(&h->d_y, rows * H * sizeof(float)));
   CU_OR_BAIL(cudaMalloc(&h->d_clk, 4 * sizeof(unsigned long long)));
+  CU_OR_BAIL(cudaMalloc(&h->d_sched, 2 * sizeof(int)));
   CU_OR_BAIL(cudaMalloc(&h->d_err, sizeof(int)));
   CU_OR_BAIL(cudaMemset(h->d_err, 0, sizeof(int)));
   // padding rows are read by the tensor cores (their outputs are discarded): keep them finite
@@ -637,6 +648,8 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
   CU_OR_BAIL(cudaFuncSetAttribute(slp::tc::gemm_tc_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::tc::Cfg<1, true>::kSmemBytes));
   CU_OR_BAIL(cudaFuncSetAttribute(slp::tc::gemm_tc_kernel<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::tc::Cfg<0, false>::kSmemBytes));
   CU_OR_BAIL(cudaFuncSetAttribute(slp::tc::gemm_tc_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::tc::Cfg<1, false>::kSmemBytes));
+  CU_OR_BAIL(cudaFuncSetAttribute(slp::tc::gemm_tc_kernel<0, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::tc::Cfg<0, false>::kSmemBytes));
+  CU_OR_BAIL(cudaFuncSetAttribute(slp::tc::gemm_tc_kernel<1, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::tc::Cfg<1, false>::kSmemBytes));
   CU_OR_BAIL(cudaDeviceSynchronize());
 #undef TRY_OR_BAIL
 #undef CU_OR_BAIL
@@ -723,7 +736,7 @@ slp_status slp_moe_layer_destroy(slp_moe_layer* h) {
   free_pool(h);
   void* ptrs[] = {h->d_router_hl, h->d_router_w, h->d_bias, h->d_gate_s, h->d_up_s, h->d_down_s, h->d_logits, h->d_w, h->d_xs, h->d_hs, h->d_idx,
                   h->d_counts, h->d_chunk, h->d_row_start, h->d_tile_start, h->d_tile_expert, h->d_pair_start, h->d_pair_expert, h->d_tile_info, h->d_pos, h->d_row_token, h->d_xq,
-                  h->d_hq, h->d_y, h->d_err, h->d_clk, h->d_e2e_in, h->d_e2e_out};
+                  h->d_hq, h->d_y, h->d_err, h->d_clk, h->d_sched, h->d_e2e_in, h->d_e2e_out};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   if (h->h_counts) cudaFreeHost(h->h_counts);

@@ -114,7 +114,7 @@ def test_layer_parity_simt(name, mode):
 @pytest.mark.parametrize("name", list(CASES))
 @pytest.mark.parametrize("mode", ["resident", "streamed"])
 def test_layer_parity_tcgen05(name, mode):
-    """gemm_impl 0: the product path (tcgen05 / TMEM / TMA, one CTA per 128 x 256 tile)."""
+    """gemm_impl 0: the product path (tcgen05 / TMEM / TMA, one CTA per 128 x 256 tile, dynamic tile order)."""
     check(name, mode, gemm_impl=0)
 
 
@@ -125,8 +125,15 @@ def test_layer_parity_tcgen05_cta_pair(name):
     check(name, "resident", gemm_impl=2)
 
 
+@pytest.mark.parametrize("name", list(CASES))
+@pytest.mark.parametrize("mode", ["resident", "streamed"])
+def test_layer_parity_tcgen05_static_tiles(name, mode):
+    """gemm_impl 3: the one-CTA kernel with the static round-robin tile order."""
+    check(name, mode, gemm_impl=3)
+
+
 @pytest.mark.parametrize("T", [1, 127, 128, 129, 257])
-@pytest.mark.parametrize("gemm_impl", [0, 2])
+@pytest.mark.parametrize("gemm_impl", [0, 2, 3])
 def test_ragged_token_counts(T, gemm_impl):
     """Edge sizes: a single token, one row short of / exactly / one row past a 128-row tile."""
     cfg, W, hidden, _ = problem("mini_dsv3")
