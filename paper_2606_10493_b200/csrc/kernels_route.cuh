@@ -344,26 +344,40 @@ __device__ __forceinline__ uint32_t quant4_e4m3(float a, float b, float c, float
 __global__ void __launch_bounds__(256) quant_scatter_kernel(const uint16_t* __restrict__ x, const int32_t* __restrict__ pos,
                                                             uint8_t* __restrict__ xq, float* __restrict__ xs, int T, int H, int k,
                                                             int xs_stride) {
+  // One block per token; a half-warp owns a 128-channel block (8 channels = one 16-byte load per lane),
+  // so a warp quantises two blocks per step: half the instructions per byte of a lane-per-4-channels
+  // layout (the kernel is issue-bound on the IEEE divisions, not on HBM).
   const int t = blockIdx.x;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
+  const int sub = lane >> 4, l16 = lane & 15;
   __shared__ int32_t dst[33];
   if (threadIdx.x < k) dst[threadIdx.x + 1] = pos[static_cast<size_t>(t) * k + threadIdx.x];
   if (threadIdx.x == 0) dst[0] = t;
   __syncthreads();
   const int nkb = H / kBlock;
-  for (int kb = warp; kb < nkb; kb += nwarps) {
-    const uint2 raw = *reinterpret_cast<const uint2*>(x + static_cast<size_t>(t) * H + kb * kBlock + lane * 4);
-    const float a = bf16_bits_to_float(raw.x & 0xFFFF), b = bf16_bits_to_float(raw.x >> 16);
-    const float c = bf16_bits_to_float(raw.y & 0xFFFF), d = bf16_bits_to_float(raw.y >> 16);
-    float amax = fmaxf(fmaxf(fabsf(a), fabsf(b)), fmaxf(fabsf(c), fabsf(d)));
+  for (int kb0 = warp * 2; kb0 < nkb; kb0 += nwarps * 2) {
+    const int kb = kb0 + sub;
+    const bool on = kb < nkb;  // odd number of blocks: the upper half-warp idles in the last step
+    uint4 raw = make_uint4(0u, 0u, 0u, 0u);
+    if (on) raw = *reinterpret_cast<const uint4*>(x + static_cast<size_t>(t) * H + kb * kBlock + l16 * 8);
+    float v[8];
+    v[0] = bf16_bits_to_float(raw.x & 0xFFFF); v[1] = bf16_bits_to_float(raw.x >> 16);
+    v[2] = bf16_bits_to_float(raw.y & 0xFFFF); v[3] = bf16_bits_to_float(raw.y >> 16);
+    v[4] = bf16_bits_to_float(raw.z & 0xFFFF); v[5] = bf16_bits_to_float(raw.z >> 16);
+    v[6] = bf16_bits_to_float(raw.w & 0xFFFF); v[7] = bf16_bits_to_float(raw.w >> 16);
+    float amax = 0.f;
 #pragma unroll
-    for (int off = 16; off > 0; off >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xFFFFFFFFu, amax, off));
+    for (int i = 0; i < 8; ++i) amax = fmaxf(amax, fabsf(v[i]));
+#pragma unroll
+    for (int off = 8; off > 0; off >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xFFFFFFFFu, amax, off));  // within the half-warp
     const float s = (amax == 0.f) ? 1.0f : __fdiv_rn(amax, 448.0f);
-    const uint32_t q = quant4_e4m3(a, b, c, d, s);
-    for (int j = 0; j <= k; ++j) {
-      const size_t row = dst[j];
-      *reinterpret_cast<uint32_t*>(xq + row * H + kb * kBlock + lane * 4) = q;
-      if (lane == 0) xs[row * xs_stride + kb] = s;
+    const uint2 q = make_uint2(quant4_e4m3(v[0], v[1], v[2], v[3], s), quant4_e4m3(v[4], v[5], v[6], v[7], s));
+    if (on) {
+      for (int j = 0; j <= k; ++j) {
+        const size_t row = dst[j];
+        *reinterpret_cast<uint2*>(xq + row * H + kb * kBlock + l16 * 8) = q;
+        if (l16 == 0) xs[row * xs_stride + kb] = s;
+      }
     }
   }
 }
