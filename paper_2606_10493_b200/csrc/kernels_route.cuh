@@ -208,6 +208,125 @@ __global__ void __launch_bounds__(256) router_topk_kernel(const float* __restric
   }
 }
 
+// Same selection for the common layouts (E = 32 * kP, n_group a power of two <= 32): lane l holds the
+// kP CONTIGUOUS experts l*kP .. l*kP+kP-1, so an expert group is a run of 32 / G lanes and all G
+// group scores (sum of the two best sel of the group) come out of log2(32 / G) shuffle steps at once
+// instead of G full-warp reductions; the kept groups follow from each group's rank among the G
+// scores (ties to the lower group, as the iterative arg-max of the general kernel).  Identical
+// results: same score formulas, same tie-breaks, same order of the weight sum.
+template <int kP>
+__global__ void __launch_bounds__(256) router_topk_fast_kernel(const float* __restrict__ logits, const float* __restrict__ bias,
+                                                               int32_t* __restrict__ idx, float* __restrict__ wout, int T, int k,
+                                                               int G, int Gk, int scoring, int norm_topk, float scale) {
+  constexpr int E = 32 * kP;
+  const int lane = threadIdx.x & 31;
+  const int t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (t >= T) return;
+  const float NEG = -INFINITY;
+  const int e0 = lane * kP;
+  float s[kP], sel[kP];
+  {
+    const float* row = logits + static_cast<size_t>(t) * E + e0;
+    if (kP % 4 == 0) {
+#pragma unroll
+      for (int r = 0; r < kP; r += 4) {
+        const float4 v = *reinterpret_cast<const float4*>(row + r);
+        s[r] = v.x; s[r + 1 < kP ? r + 1 : r] = v.y; s[r + 2 < kP ? r + 2 : r] = v.z; s[r + 3 < kP ? r + 3 : r] = v.w;
+      }
+    } else {
+#pragma unroll
+      for (int r = 0; r < kP; ++r) s[r] = row[r];
+    }
+  }
+  if (scoring == 0) {
+#pragma unroll
+    for (int r = 0; r < kP; ++r) {
+      const float sc = 1.0f / (1.0f + expf(-s[r]));
+      s[r] = sc;
+      sel[r] = sc + (bias ? bias[e0 + r] : 0.0f);
+    }
+  } else {
+    float lmax = NEG;
+#pragma unroll
+    for (int r = 0; r < kP; ++r) lmax = fmaxf(lmax, s[r]);
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) lmax = fmaxf(lmax, __shfl_xor_sync(0xFFFFFFFFu, lmax, off));
+    float z = 0.f;
+#pragma unroll
+    for (int r = 0; r < kP; ++r) {
+      sel[r] = s[r];                 // select by logit
+      s[r] = expf(s[r] - lmax);      // unnormalised probability
+      z += s[r];
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) z += __shfl_xor_sync(0xFFFFFFFFu, z, off);
+    if (!norm_topk) {
+      const float inv = 1.0f / z;
+#pragma unroll
+      for (int r = 0; r < kP; ++r) s[r] *= inv;
+    }
+  }
+
+  if (G > 1) {
+    const int lpg = 32 / G;  // lanes per group
+    float m1 = NEG, m2 = NEG;
+#pragma unroll
+    for (int r = 0; r < kP; ++r) {
+      const float v = sel[r];
+      if (v > m1) { m2 = m1; m1 = v; } else if (v > m2) { m2 = v; }
+    }
+    for (int off = lpg >> 1; off > 0; off >>= 1) {
+      const float o1 = __shfl_xor_sync(0xFFFFFFFFu, m1, off);
+      const float o2 = __shfl_xor_sync(0xFFFFFFFFu, m2, off);
+      const float n1 = fmaxf(m1, o1);
+      const float n2 = fmaxf(fminf(m1, o1), fmaxf(m2, o2));
+      m1 = n1; m2 = n2;
+    }
+    const float gsc = (kP * lpg >= 2) ? (m1 + m2) : m1;  // every lane of a group now holds its score
+    const int g = lane / lpg;
+    int rank = 0;
+    for (int o = 0; o < G; ++o) {
+      const float os = __shfl_sync(0xFFFFFFFFu, gsc, o * lpg);
+      rank += (os > gsc || (os == gsc && o < g)) ? 1 : 0;
+    }
+    if (rank >= Gk) {
+#pragma unroll
+      for (int r = 0; r < kP; ++r) sel[r] = NEG;
+    }
+  }
+
+  float my_w = 0.f;
+  int my_e = 0;
+  float wsum = 0.f;
+  for (int j = 0; j < k; ++j) {
+    float bv = NEG;
+    int br = 0;
+#pragma unroll
+    for (int r = 0; r < kP; ++r) {  // ascending index, strict >: ties to the lower expert
+      const bool better = sel[r] > bv;
+      bv = better ? sel[r] : bv;
+      br = better ? r : br;
+    }
+    // an all-excluded lane offers (-inf, its first expert); a real candidate always beats it or ties with a lower index
+    const ArgMax a = warp_argmax(bv, e0 + br);
+    float sc = 0.f;
+#pragma unroll
+    for (int r = 0; r < kP; ++r) {
+      const bool hit = e0 + r == a.i;
+      sc = hit ? s[r] : sc;
+      sel[r] = hit ? NEG : sel[r];
+    }
+    sc = __shfl_sync(0xFFFFFFFFu, sc, a.i / kP);
+    wsum += sc;
+    if (lane == j) { my_w = sc; my_e = a.i; }
+  }
+  if (lane < k) {
+    const float wv = norm_topk ? my_w / wsum : my_w;
+    idx[static_cast<size_t>(t) * k + lane] = my_e;
+    wout[static_cast<size_t>(t) * k + lane] = wv * scale;
+  }
+}
+
 // ---------------------------------------------------------------------------------------------
 // a2: histogram / scan / permute.  Workspace rows: [0, Tpad) hold the un-permuted tokens (the
 // shared expert's rows), then each routed expert owns a 128-aligned row range holding its tokens

@@ -368,6 +368,23 @@ slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t
     const int warps = 8;
     const int blocks = (T + warps - 1) / warps;
     const float* bias = h->cfg.scoring == SLP_SCORE_SIGMOID_BIAS ? h->d_bias : nullptr;
+    const int G = h->cfg.n_group;
+    const bool fast = E % 32 == 0 && (E / 32 == 1 || E / 32 == 2 || E / 32 == 4 || E / 32 == 8 || E / 32 == 16) &&
+                      (G & (G - 1)) == 0 && G <= 32;
+#define SLP_TOPK_FAST(P)                                                                                              \
+  slp::router_topk_fast_kernel<P><<<blocks, warps * 32, 0, s>>>(h->d_logits, bias, h->d_idx, h->d_w, T, k, G,         \
+                                                                h->cfg.topk_group, h->cfg.scoring, h->cfg.norm_topk, \
+                                                                h->cfg.routed_scale)
+    if (fast) {  // contiguous experts per lane: groups are runs of lanes (kernels_route.cuh)
+      switch (E / 32) {
+        case 1: SLP_TOPK_FAST(1); break;
+        case 2: SLP_TOPK_FAST(2); break;
+        case 4: SLP_TOPK_FAST(4); break;
+        case 8: SLP_TOPK_FAST(8); break;
+        default: SLP_TOPK_FAST(16); break;
+      }
+    } else
+#undef SLP_TOPK_FAST
     if (E <= 128)
       slp::router_topk_kernel<4><<<blocks, warps * 32, 0, s>>>(h->d_logits, bias, h->d_idx, h->d_w, T, E, k, h->cfg.n_group,
                                                                h->cfg.topk_group, h->cfg.scoring, h->cfg.norm_topk, h->cfg.routed_scale);
