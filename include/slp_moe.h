@@ -134,6 +134,24 @@ typedef struct {
   float sm_mhz_down;          /* same for the down launches */
 } slp_moe_stats;
 
+/* What create would allocate and how prefill would launch for a configuration (host arithmetic only). */
+typedef struct {
+  uint32_t struct_size;            /* = sizeof(slp_moe_plan) */
+  int32_t staging_slots;           /* expert slots of the streamed ring after defaults (0 -> n_experts) */
+  int32_t experts_per_launch;      /* experts per grouped-GEMM launch pair after defaults */
+  int32_t launch_pairs_streamed;   /* gate/up + down launch pairs per streamed call (incl. the shared expert) */
+  int64_t workspace_rows;          /* rows of xq / hq / Y: padded tokens + 128-aligned expert ranges */
+  int64_t expert_slot_bytes;       /* 3 * I * H: gate | up | down of one expert ("3 FP8 linears") */
+  int64_t routed_bytes_per_pass;   /* E * 3 * I * H: what one streamed call moves over the host link */
+  int64_t pool_bytes_streamed;     /* (1 + staging_slots) slots */
+  int64_t pool_bytes_resident;     /* (1 + E) slots */
+  int64_t scale_bytes;             /* resident fp32 block scales of all experts */
+  int64_t workspace_bytes;         /* activations and routing tables for max_tokens (approximate total) */
+  int64_t fp8_flops_per_token;     /* 2 * 3 * I * H * (top_k + n_shared) */
+  int32_t gemm_smem_bytes_gateup;  /* dynamic shared memory of the grouped-GEMM kernels */
+  int32_t gemm_smem_bytes_down;
+} slp_moe_plan;
+
 /* Buffers readable through slp_moe_debug_buffer (parity / evidence; layouts in DESIGN.md §5). */
 typedef enum {
   SLP_BUF_COUNTS = 0,      /* int32 [E] tokens per routed expert */
@@ -150,6 +168,10 @@ typedef enum {
  * tensors, allocates workspace for cfg->max_tokens and the expert slots.  Starts in SLP_STREAMED.
  * Errors: INVALID_ARG (NULL / bad struct_size), UNSUPPORTED_SHAPE, NOT_PINNED, OOM, CUDA. */
 slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weights* w, slp_moe_layer** out);
+
+/* Validates cfg exactly as create does and fills *plan; needs no GPU and allocates nothing.
+ * Errors: INVALID_ARG, UNSUPPORTED_SHAPE (same messages as create). */
+slp_status slp_moe_query_plan(const slp_moe_cfg* cfg, slp_moe_plan* plan);
 
 /* Switch residency.  SLP_RESIDENT uploads all E experts into HBM once (blocking) and later calls
  * copy nothing; SLP_STREAMED frees that copy and returns to per-call streaming.  Blocks until the

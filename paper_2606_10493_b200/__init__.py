@@ -8,5 +8,5 @@ PyTorch fallback for any step of the path.
 
 from . import inputs, sharding  # noqa: F401
 from .binding import (  # noqa: F401
-    SlpMoeLayer, SlpError, lib, library_path, measure_h2d_gbs, EXPORTED_SYMBOLS,
+    SlpMoeLayer, SlpError, lib, library_path, measure_h2d_gbs, query_plan, EXPORTED_SYMBOLS,
 )

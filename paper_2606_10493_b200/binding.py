@@ -15,7 +15,7 @@ EXPORTED_SYMBOLS = [
     "slp_moe_layer_create", "slp_moe_set_residency", "slp_moe_prefill", "slp_moe_prefill_host",
     "slp_moe_layer_destroy", "slp_last_error", "slp_moe_debug_routing",
     "slp_moe_debug_quant_hidden", "slp_moe_debug_buffer", "slp_moe_get_stats",
-    "slp_measure_h2d", "slp_version",
+    "slp_measure_h2d", "slp_version", "slp_moe_query_plan",
 ]
 
 SLP_STREAMED, SLP_RESIDENT = 0, 1
@@ -116,6 +116,39 @@ def _ptr_array(tensor):
     return arr
 
 
+class Plan(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("staging_slots", C.c_int32), ("experts_per_launch", C.c_int32),
+                ("launch_pairs_streamed", C.c_int32), ("workspace_rows", C.c_int64),
+                ("expert_slot_bytes", C.c_int64), ("routed_bytes_per_pass", C.c_int64),
+                ("pool_bytes_streamed", C.c_int64), ("pool_bytes_resident", C.c_int64),
+                ("scale_bytes", C.c_int64), ("workspace_bytes", C.c_int64), ("fp8_flops_per_token", C.c_int64),
+                ("gemm_smem_bytes_gateup", C.c_int32), ("gemm_smem_bytes_down", C.c_int32)]
+
+    def as_dict(self):
+        return {n: getattr(self, n) for n, _ in self._fields_ if n != "struct_size"}
+
+
+def _make_cfg(cfg, *, max_tokens=None, device=0, staging_slots=0, experts_per_launch=0, skip_empty_experts=False,
+              require_pinned=False, gemm_impl=0, router_impl=0):
+    return _Cfg(struct_size=C.sizeof(_Cfg), device=device, hidden=cfg.H, n_experts=cfg.E,
+                top_k=cfg.k, n_group=cfg.G, topk_group=cfg.Gk, moe_intermediate=cfg.I,
+                n_shared=cfg.n_shared, shared_intermediate=cfg.I if cfg.n_shared else 0,
+                scoring=SCORING[cfg.scoring], norm_topk=int(cfg.norm_topk),
+                routed_scale=cfg.routed_scale, max_tokens=max_tokens or cfg.T,
+                staging_slots=staging_slots, experts_per_launch=experts_per_launch,
+                skip_empty_experts=int(skip_empty_experts), require_pinned=int(require_pinned),
+                gemm_impl=gemm_impl, router_impl=router_impl)
+
+
+def query_plan(cfg, **kw):
+    """slp_moe_query_plan: validates the configuration as create does and returns what would be
+    allocated / launched (host arithmetic only, no GPU needed).  Raises SlpError on a bad shape."""
+    c = _make_cfg(cfg, **kw)
+    plan = Plan(struct_size=C.sizeof(Plan))
+    _check(lib().slp_moe_query_plan(C.byref(c), C.byref(plan)))
+    return plan.as_dict()
+
+
 class SlpMoeLayer:
     """One MoE layer handle.  `weights` is the dict `inputs.make_weights` returns (host torch
     tensors, kept alive by this object because the library borrows the memory)."""
@@ -126,14 +159,9 @@ class SlpMoeLayer:
         self.cfg = cfg
         self.weights = weights
         self.max_tokens = max_tokens or cfg.T
-        c = _Cfg(struct_size=C.sizeof(_Cfg), device=device, hidden=cfg.H, n_experts=cfg.E,
-                 top_k=cfg.k, n_group=cfg.G, topk_group=cfg.Gk, moe_intermediate=cfg.I,
-                 n_shared=cfg.n_shared, shared_intermediate=cfg.I if cfg.n_shared else 0,
-                 scoring=SCORING[cfg.scoring], norm_topk=int(cfg.norm_topk),
-                 routed_scale=cfg.routed_scale, max_tokens=self.max_tokens,
-                 staging_slots=staging_slots, experts_per_launch=experts_per_launch,
-                 skip_empty_experts=int(skip_empty_experts), require_pinned=int(require_pinned),
-                 gemm_impl=gemm_impl, router_impl=router_impl)
+        c = _make_cfg(cfg, max_tokens=self.max_tokens, device=device, staging_slots=staging_slots,
+                      experts_per_launch=experts_per_launch, skip_empty_experts=skip_empty_experts,
+                      require_pinned=require_pinned, gemm_impl=gemm_impl, router_impl=router_impl)
         w = weights
         self._arrays = {k: _ptr_array(w[k]) for k in ("gate_q", "gate_s", "up_q", "up_s", "down_q", "down_s")}
 

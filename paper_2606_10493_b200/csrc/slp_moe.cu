@@ -105,6 +105,34 @@ inline int auto_epl(int n_stage, int E) {
 
 inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
 
+// Shape / option validation shared by create and slp_moe_query_plan (no CUDA calls).  On success
+// *n_stage = expert slots of the streamed ring, *epl = experts per grouped-GEMM launch.
+slp_status validate_cfg(const slp_moe_cfg* cfg, int* n_stage_out, int* epl_out) {
+  const int H = cfg->hidden, E = cfg->n_experts, k = cfg->top_k, I = cfg->moe_intermediate, G = cfg->n_group, Gk = cfg->topk_group;
+  if (H <= 0 || I <= 0 || H % 128 || I % 128 || H / 128 > 1024 || I / 128 > 1024)
+    return fail(SLP_ERR_UNSUPPORTED_SHAPE, "hidden (%d) and moe_intermediate (%d) must be positive multiples of 128", H, I);
+  if (E <= 0 || E > slp::kMaxExperts - 1) return fail(SLP_ERR_UNSUPPORTED_SHAPE, "n_experts %d outside 1..%d", E, slp::kMaxExperts - 1);
+  if (G <= 0 || G > 32 || E % G || Gk <= 0 || Gk > G) return fail(SLP_ERR_UNSUPPORTED_SHAPE, "n_group %d / topk_group %d invalid for %d experts", G, Gk, E);
+  if (k <= 0 || k > 32 || k > E || static_cast<long long>(k) > static_cast<long long>(Gk) * (E / G))
+    return fail(SLP_ERR_UNSUPPORTED_SHAPE, "top_k %d invalid (needs 1..32, <= topk_group * E / n_group)", k);
+  if (cfg->n_shared < 0 || cfg->n_shared > 1 || (cfg->n_shared == 1 && cfg->shared_intermediate != I))
+    return fail(SLP_ERR_UNSUPPORTED_SHAPE, "n_shared must be 0 or 1 with shared_intermediate == moe_intermediate");
+  if (cfg->scoring != SLP_SCORE_SIGMOID_BIAS && cfg->scoring != SLP_SCORE_SOFTMAX) return fail(SLP_ERR_INVALID_ARG, "unknown scoring %d", cfg->scoring);
+  if (cfg->max_tokens <= 0) return fail(SLP_ERR_INVALID_ARG, "max_tokens must be positive");
+  if (cfg->gemm_impl < 0 || cfg->gemm_impl > 3) return fail(SLP_ERR_INVALID_ARG, "gemm_impl must be 0, 1, 2 or 3");
+  if (cfg->router_impl != 0 && cfg->router_impl != 1) return fail(SLP_ERR_INVALID_ARG, "router_impl must be 0 or 1");
+  int n_stage = cfg->staging_slots == 0 ? E : cfg->staging_slots;
+  if (n_stage < 2 && E >= 2) return fail(SLP_ERR_INVALID_ARG, "staging_slots must be 0 or 2..n_experts");
+  n_stage = std::min(n_stage, E);
+  int epl = cfg->experts_per_launch;
+  if (epl == 0) epl = auto_epl(n_stage, E);
+  if (epl < 1 || epl > n_stage || (n_stage != E && (epl > n_stage / 2 || n_stage % epl)))
+    return fail(SLP_ERR_INVALID_ARG, "experts_per_launch %d invalid for %d staging slots (must divide it, <= half)", epl, n_stage);
+  *n_stage_out = n_stage;
+  *epl_out = epl;
+  return SLP_OK;
+}
+
 }  // namespace
 
 struct slp_moe_layer {
@@ -502,26 +530,12 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
   if (!cfg || !w || !out) return fail(SLP_ERR_INVALID_ARG, "NULL argument");
   if (cfg->struct_size != sizeof(slp_moe_cfg)) return fail(SLP_ERR_INVALID_ARG, "cfg.struct_size %u != %zu", cfg->struct_size, sizeof(slp_moe_cfg));
   *out = nullptr;
-  const int H = cfg->hidden, E = cfg->n_experts, k = cfg->top_k, I = cfg->moe_intermediate, G = cfg->n_group, Gk = cfg->topk_group;
-  if (H <= 0 || I <= 0 || H % 128 || I % 128 || H / 128 > 1024 || I / 128 > 1024)
-    return fail(SLP_ERR_UNSUPPORTED_SHAPE, "hidden (%d) and moe_intermediate (%d) must be positive multiples of 128", H, I);
-  if (E <= 0 || E > slp::kMaxExperts - 1) return fail(SLP_ERR_UNSUPPORTED_SHAPE, "n_experts %d outside 1..%d", E, slp::kMaxExperts - 1);
-  if (G <= 0 || G > 32 || E % G || Gk <= 0 || Gk > G) return fail(SLP_ERR_UNSUPPORTED_SHAPE, "n_group %d / topk_group %d invalid for %d experts", G, Gk, E);
-  if (k <= 0 || k > 32 || k > E || static_cast<long long>(k) > static_cast<long long>(Gk) * (E / G))
-    return fail(SLP_ERR_UNSUPPORTED_SHAPE, "top_k %d invalid (needs 1..32, <= topk_group * E / n_group)", k);
-  if (cfg->n_shared < 0 || cfg->n_shared > 1 || (cfg->n_shared == 1 && cfg->shared_intermediate != I))
-    return fail(SLP_ERR_UNSUPPORTED_SHAPE, "n_shared must be 0 or 1 with shared_intermediate == moe_intermediate");
-  if (cfg->scoring != SLP_SCORE_SIGMOID_BIAS && cfg->scoring != SLP_SCORE_SOFTMAX) return fail(SLP_ERR_INVALID_ARG, "unknown scoring %d", cfg->scoring);
-  if (cfg->max_tokens <= 0) return fail(SLP_ERR_INVALID_ARG, "max_tokens must be positive");
-  if (cfg->gemm_impl < 0 || cfg->gemm_impl > 3) return fail(SLP_ERR_INVALID_ARG, "gemm_impl must be 0, 1, 2 or 3");
-  if (cfg->router_impl != 0 && cfg->router_impl != 1) return fail(SLP_ERR_INVALID_ARG, "router_impl must be 0 or 1");
-  int n_stage = cfg->staging_slots == 0 ? E : cfg->staging_slots;
-  if (n_stage < 2 && E >= 2) return fail(SLP_ERR_INVALID_ARG, "staging_slots must be 0 or 2..n_experts");
-  n_stage = std::min(n_stage, E);
-  int epl = cfg->experts_per_launch;
-  if (epl == 0) epl = auto_epl(n_stage, E);
-  if (epl < 1 || epl > n_stage || (n_stage != E && (epl > n_stage / 2 || n_stage % epl)))
-    return fail(SLP_ERR_INVALID_ARG, "experts_per_launch %d invalid for %d staging slots (must divide it, <= half)", epl, n_stage);
+  const int H = cfg->hidden, E = cfg->n_experts, k = cfg->top_k, I = cfg->moe_intermediate;
+  int n_stage = 0, epl = 0;
+  {
+    slp_status vst = validate_cfg(cfg, &n_stage, &epl);
+    if (vst != SLP_OK) return vst;
+  }
   if (!w->router_w || !w->gate_q || !w->gate_s || !w->up_q || !w->up_s || !w->down_q || !w->down_s)
     return fail(SLP_ERR_INVALID_ARG, "NULL weight pointer");
   if (cfg->n_shared && (!w->shared_gate_q || !w->shared_gate_s || !w->shared_up_q || !w->shared_up_s || !w->shared_down_q || !w->shared_down_s))
@@ -671,6 +685,33 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
 #undef TRY_OR_BAIL
 #undef CU_OR_BAIL
   *out = h;
+  return SLP_OK;
+}
+
+slp_status slp_moe_query_plan(const slp_moe_cfg* cfg, slp_moe_plan* plan) {
+  if (!cfg || !plan) return fail(SLP_ERR_INVALID_ARG, "NULL argument");
+  if (cfg->struct_size != sizeof(slp_moe_cfg)) return fail(SLP_ERR_INVALID_ARG, "cfg.struct_size %u != %zu", cfg->struct_size, sizeof(slp_moe_cfg));
+  if (plan->struct_size != sizeof(slp_moe_plan)) return fail(SLP_ERR_INVALID_ARG, "plan.struct_size mismatch");
+  int n_stage = 0, epl = 0;
+  slp_status st = validate_cfg(cfg, &n_stage, &epl);
+  if (st != SLP_OK) return st;
+  const int64_t H = cfg->hidden, E = cfg->n_experts, k = cfg->top_k, I = cfg->moe_intermediate, Tm = cfg->max_tokens;
+  const int64_t Tpad = (Tm + 127) / 128 * 128;
+  const int64_t rows = Tpad + (Tm * k + E * 127 + 127) / 128 * 128;
+  const int64_t xs_stride = (H / 128 + 3) / 4 * 4, hs_stride = (I / 128 + 3) / 4 * 4;
+  plan->staging_slots = n_stage;
+  plan->experts_per_launch = epl;
+  plan->launch_pairs_streamed = static_cast<int32_t>((E + epl - 1) / epl + (cfg->n_shared ? 1 : 0));
+  plan->workspace_rows = rows;
+  plan->expert_slot_bytes = 3 * I * H;
+  plan->routed_bytes_per_pass = E * 3 * I * H;
+  plan->pool_bytes_streamed = (1 + n_stage) * 3 * I * H;
+  plan->pool_bytes_resident = (1 + E) * 3 * I * H;
+  plan->scale_bytes = (E + 1) * (2 * (I / 128) * (H / 128) + (H / 128) * (I / 128)) * 4;
+  plan->workspace_bytes = rows * (H + xs_stride * 4 + I + hs_stride * 4 + H * 4 + 4) + Tm * (E * 4 + k * 12);
+  plan->fp8_flops_per_token = 2 * 3 * I * H * (k + cfg->n_shared);
+  plan->gemm_smem_bytes_gateup = slp::tc::Cfg<0, false>::kSmemBytes;
+  plan->gemm_smem_bytes_down = slp::tc::Cfg<1, false>::kSmemBytes;
   return SLP_OK;
 }
 

@@ -67,3 +67,59 @@ def test_shape_validation_precedes_device_use(built):
         with pytest.raises(SlpError) as ei:
             SlpMoeLayer(inputs.LayerConfig(**{**cfg.__dict__, **bad}), W)
         assert ei.value.status == -2, bad
+
+
+# ---- host logic reachable without a GPU: slp_moe_query_plan (same validation as create) ----------
+
+def _cfg(**kw):
+    from paper_2606_10493_b200 import inputs
+    return inputs.LayerConfig(**{**inputs.CONFIGS[1].__dict__, **kw})
+
+
+def test_query_plan_byte_accounting_matches_the_paper(built):
+    """PAPER.md:412 "11.3 GB" of routed FP8 weights per DeepSeek-V3 layer; PAPER.md:140 one ring slot
+    = one expert's three FP8 linears (44.5 K tensors = 58 x 256 x 3)."""
+    from paper_2606_10493_b200 import inputs
+    p = binding.query_plan(inputs.CONFIGS[1])
+    assert p["expert_slot_bytes"] == 3 * 2048 * 7168 == 44040192
+    assert p["routed_bytes_per_pass"] == 11274289152 and round(p["routed_bytes_per_pass"] / 1e9, 1) == 11.3
+    assert p["staging_slots"] == 256 and p["pool_bytes_streamed"] == 257 * 44040192 == p["pool_bytes_resident"]
+    assert p["experts_per_launch"] == 64 and p["launch_pairs_streamed"] == 4 + 1
+    assert p["scale_bytes"] == 257 * 3 * 16 * 56 * 4
+    assert p["fp8_flops_per_token"] == 2 * 3 * 2048 * 7168 * 9 == inputs.fp8_flops_per_token(inputs.CONFIGS[1])
+    assert p["workspace_rows"] == 4096 + (4096 * 8 + 256 * 127 + 127) // 128 * 128
+    assert max(p["gemm_smem_bytes_gateup"], p["gemm_smem_bytes_down"]) <= 227 * 1024
+    k2 = binding.query_plan(_cfg(E=384, G=8, Gk=4))            # Kimi-K2-like expert count: "16.9 GB" (PAPER.md:412)
+    assert round(k2["routed_bytes_per_pass"] / 1e9, 1) == 16.9
+
+
+def test_query_plan_ring_defaults(built):
+    from paper_2606_10493_b200 import inputs
+    cfg = inputs.CONFIGS[1]
+    assert binding.query_plan(cfg, staging_slots=2)["experts_per_launch"] == 1          # ping-pong (PAPER.md:142)
+    p = binding.query_plan(cfg, staging_slots=96)
+    assert p["staging_slots"] == 96 and p["experts_per_launch"] == 32 and p["pool_bytes_streamed"] == 97 * 44040192
+    assert binding.query_plan(cfg, staging_slots=100)["experts_per_launch"] == 25      # largest divisor <= min(32, n/2)
+    assert binding.query_plan(cfg, staging_slots=8, experts_per_launch=4)["launch_pairs_streamed"] == 64 + 1
+    assert binding.query_plan(inputs.CONFIGS[0])["experts_per_launch"] == 8             # whole tiny layer in one launch
+
+
+@pytest.mark.parametrize("kw, status", [
+    (dict(H=7000), -2), (dict(I=100), -2), (dict(E=600), -2), (dict(E=250), -2),        # shapes
+    (dict(G=3), -2), (dict(Gk=9), -2), (dict(k=33), -2), (dict(k=200), -2), (dict(G=8, Gk=1, k=40), -2),
+    (dict(n_shared=2), -2),
+])
+def test_query_plan_rejects_unsupported_shapes(built, kw, status):
+    with pytest.raises(binding.SlpError) as ei:
+        binding.query_plan(_cfg(**kw))
+    assert ei.value.status == status and str(ei.value)
+
+
+def test_query_plan_rejects_bad_options(built):
+    from paper_2606_10493_b200 import inputs
+    cfg = inputs.CONFIGS[1]
+    for kw in (dict(staging_slots=1), dict(staging_slots=8, experts_per_launch=8), dict(staging_slots=9, experts_per_launch=2),
+               dict(gemm_impl=7), dict(router_impl=2), dict(max_tokens=-5)):
+        with pytest.raises(binding.SlpError) as ei:
+            binding.query_plan(cfg, **kw)
+        assert ei.value.status == -1, kw
