@@ -258,6 +258,11 @@ def main():
                     "peak_source": f"hbm copy {peaks['source']}"}
     roofline["frac"] = roofline["achieved"] / roofline["peak"]
     roofline["traffic"] = NCU_TRAFFIC_BYTES.get(args.workload)
+    # the ncu capture is of ONE launch: the whole layer in resident mode, one group of experts_per_launch
+    # routed experts in streamed mode; the algorithmic bytes of that same launch, for comparison
+    from paper_2606_10493_b200 import query_plan
+    epl = query_plan(cfg, staging_slots=args.staging_slots, experts_per_launch=args.experts_per_launch)["experts_per_launch"]
+    roofline["traffic_launch_algorithmic_bytes"] = gu_bytes if mode == "resident" else gu_bytes * min(epl, cfg.E) / max(1, n_exp_run)
     roofline["algorithmic_bytes_per_launch"] = gu_bytes / max(1, st["timed_gemm_pairs"])
     roofline["algorithmic_flops_per_launch"] = gu_flops / max(1, st["timed_gemm_pairs"])
     roofline["ms_per_launch"] = gu_ms
