@@ -473,7 +473,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
         }
         float* ex = reinterpret_cast<float*>(scratch) + tile_parity * 2 * BM;  // [parity][half][row]
         ex[half * BM + r_in_tile] = amax;
-        ptx::named_bar_sync(1, kEpiWarps * 32);
+        ptx::named_bar_sync(1 + q, 64);  // only the two warps that share these 32 rows (w and w + 4) meet
         amax = fmaxf(amax, ex[(half ^ 1) * BM + r_in_tile]);
         const float s = (amax == 0.f) ? 1.0f : __fdiv_rn(amax, 448.0f);
         if (row_ok_cur) {
