@@ -365,12 +365,12 @@ __global__ void __launch_bounds__(512) permute_scan_kernel(int32_t* __restrict__
   const int e = threadIdx.x;
   if (e < E) {
     int run = 0;
-    for (int c0 = 0; c0 < n_chunks; c0 += 8) {  // 8 independent loads in flight, then the serial scan
-      int v[8];
+    for (int c0 = 0; c0 < n_chunks; c0 += 32) {  // 32 independent loads in flight, then the serial scan
+      int v[32];
 #pragma unroll
-      for (int u = 0; u < 8; ++u) v[u] = (c0 + u < n_chunks) ? chunk_counts[static_cast<size_t>(c0 + u) * E + e] : 0;
+      for (int u = 0; u < 32; ++u) v[u] = (c0 + u < n_chunks) ? chunk_counts[static_cast<size_t>(c0 + u) * E + e] : 0;
 #pragma unroll
-      for (int u = 0; u < 8; ++u) {
+      for (int u = 0; u < 32; ++u) {
         if (c0 + u < n_chunks) chunk_counts[static_cast<size_t>(c0 + u) * E + e] = run;
         run += v[u];
       }
