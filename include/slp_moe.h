@@ -132,6 +132,8 @@ typedef struct {
   float ms_down_sum;          /* same for the down kernel */
   float sm_mhz_gateup;        /* average SM clock during the gate/up launches (clock64 / globaltimer of CTA 0) */
   float sm_mhz_down;          /* same for the down launches */
+  int32_t h2d_copies;         /* cudaMemcpyAsync calls the streaming engine issued (consecutive experts merge) */
+  int32_t reserved;
 } slp_moe_stats;
 
 /* What create would allocate and how prefill would launch for a configuration (host arithmetic only). */

@@ -58,7 +58,8 @@ class Stats(C.Structure):
                 ("ms_route", C.c_float), ("ms_experts", C.c_float), ("ms_combine", C.c_float),
                 ("gemm_launches", C.c_int32), ("kernel_launches", C.c_int32), ("m_tiles", C.c_int32),
                 ("timed_gemm_pairs", C.c_int32), ("ms_gateup_sum", C.c_float), ("ms_down_sum", C.c_float),
-                ("sm_mhz_gateup", C.c_float), ("sm_mhz_down", C.c_float)]
+                ("sm_mhz_gateup", C.c_float), ("sm_mhz_down", C.c_float),
+                ("h2d_copies", C.c_int32), ("reserved", C.c_int32)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_ if n != "struct_size"}

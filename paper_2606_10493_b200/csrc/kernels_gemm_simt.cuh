@@ -23,11 +23,12 @@ struct GemmArgs {
   int e_begin, e_end;          // experts covered by this launch: [e_begin, e_end), E = shared
   int E, T;
   int n_stage;                 // slot of routed expert e is 1 + e % n_stage; shared expert: slot 0
+  int n_slots;                 // 1 + n_stage slots per weight kind: pool = [gate slots | up slots | down slots]
   // operands
   const uint8_t* a_q;          // [rows, K] e4m3
   const float* a_s;            // [rows, a_s_stride]
   int a_s_stride;
-  const uint8_t* pool;         // expert slots: gate [I,H] | up [I,H] | down [H,I]
+  const uint8_t* pool;         // [3][n_slots][I*H]: gate [I,H] of every slot, then up [I,H], then down [H,I]
   const float* gate_s;         // [E+1, I/128, H/128]
   const float* up_s;           // [E+1, I/128, H/128]
   const float* down_s;         // [E+1, H/128, I/128]
@@ -71,10 +72,10 @@ __global__ void __launch_bounds__(256) gemm_simt_kernel(GemmArgs g) {
   const int N = kMode == 0 ? g.I : g.H;
   const int nb = blockIdx.x;  // 128-channel block of the output
   if (nb * BC >= N) return;
-  const uint8_t* slot = g.pool + static_cast<size_t>(slot_of(g, e)) * 3 * g.I * g.H;
-  const uint8_t* B0 = kMode == 0 ? slot + static_cast<size_t>(nb) * BC * K
-                                 : slot + static_cast<size_t>(2) * g.I * g.H + static_cast<size_t>(nb) * BC * K;
-  const uint8_t* B1 = slot + static_cast<size_t>(g.I) * g.H + static_cast<size_t>(nb) * BC * K;  // up (mode 0 only)
+  // pool = [gate of all slots | up of all slots | down of all slots]
+  const size_t IH = static_cast<size_t>(g.I) * g.H, sl = slot_of(g, e);
+  const uint8_t* B0 = g.pool + ((kMode == 0 ? 0 : 2) * static_cast<size_t>(g.n_slots) + sl) * IH + static_cast<size_t>(nb) * BC * K;
+  const uint8_t* B1 = g.pool + (static_cast<size_t>(g.n_slots) + sl) * IH + static_cast<size_t>(nb) * BC * K;  // up (mode 0 only)
   const int nkb = K / kBlock, nnb = N / kBlock;
   const float* s0 = (kMode == 0 ? g.gate_s : g.down_s) + (static_cast<size_t>(e) * nnb + nb) * nkb;
   const float* s1 = g.up_s + (static_cast<size_t>(e) * nnb + nb) * nkb;

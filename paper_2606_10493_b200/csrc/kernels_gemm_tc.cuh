@@ -237,11 +237,12 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
         constexpr int kBoxes = kPair ? 2 : 4;
         int brow[kBoxes];
         if (kMode == 0) {
-          const int gate0 = slot * 3 * g.I + nt * 128;  // view [slots*3I, H]
-          if (kPair) { brow[0] = gate0 + 64 * rank; brow[1] = gate0 + g.I + 64 * rank; }
-          else { brow[0] = gate0; brow[1] = gate0 + g.I; brow[2 % kBoxes] = gate0 + 64; brow[3 % kBoxes] = gate0 + g.I + 64; }
+          // pool = [gate of all slots | up of all slots | down of all slots], viewed as [3 * slots * I, H]
+          const int gate0 = slot * g.I + nt * 128, up0 = (g.n_slots + slot) * g.I + nt * 128;
+          if (kPair) { brow[0] = gate0 + 64 * rank; brow[1] = up0 + 64 * rank; }
+          else { brow[0] = gate0; brow[1] = up0; brow[2 % kBoxes] = gate0 + 64; brow[3 % kBoxes] = up0 + 64; }
         } else {
-          const int down0 = slot * 3 * g.H + 2 * g.H + nt * BN;  // view [slots*3H, I]
+          const int down0 = (2 * g.n_slots + slot) * g.H + nt * BN;  // same pool viewed as [3 * slots * H, I]
           if (kPair) { brow[0] = down0 + 128 * rank; brow[1] = brow[0] + 64; }
           else { brow[0] = down0; brow[1] = down0 + 64; brow[2 % kBoxes] = down0 + 128; brow[3 % kBoxes] = down0 + 192; }
         }

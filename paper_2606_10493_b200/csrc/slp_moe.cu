@@ -207,12 +207,17 @@ slp_status alloc_pool(L* h, int n_stage, int epl) {
   const size_t bytes = static_cast<size_t>(1 + n_stage) * h->slot_bytes;
   CU_TRY(cudaMalloc(&h->d_pool, bytes));
   const size_t IH = static_cast<size_t>(h->I) * h->H;
+  // Pool layout: [gate of all slots | up of all slots | down of all slots], slot 0 = shared expert.
+  // Kind-major so that experts that are contiguous in host memory (stacked [E, I, H] tensors, the usual
+  // fused-MoE layout) land contiguously too and several experts travel in ONE cudaMemcpyAsync: the
+  // ~4 us gap between back-to-back 14.7 MB copies is 1.5 % of the link time (profiles/r1_h2d_chunks.md).
+  const size_t S = static_cast<size_t>(1 + n_stage);
   if (h->cfg.n_shared) {
     CU_TRY(cudaMemcpy(h->d_pool, h->hw.shared_gate_q, IH, cudaMemcpyHostToDevice));
-    CU_TRY(cudaMemcpy(h->d_pool + IH, h->hw.shared_up_q, IH, cudaMemcpyHostToDevice));
-    CU_TRY(cudaMemcpy(h->d_pool + 2 * IH, h->hw.shared_down_q, IH, cudaMemcpyHostToDevice));
+    CU_TRY(cudaMemcpy(h->d_pool + S * IH, h->hw.shared_up_q, IH, cudaMemcpyHostToDevice));
+    CU_TRY(cudaMemcpy(h->d_pool + 2 * S * IH, h->hw.shared_down_q, IH, cudaMemcpyHostToDevice));
   } else {
-    CU_TRY(cudaMemset(h->d_pool, 0, h->slot_bytes));
+    for (int kind = 0; kind < 3; ++kind) CU_TRY(cudaMemset(h->d_pool + kind * S * IH, 0, IH));
   }
   slp_status st = make_tmap_u8(&h->tm_wgu, h->d_pool, h->H, static_cast<uint64_t>(1 + n_stage) * 3 * h->I, slp::tc::kBoxRows);
   if (st != SLP_OK) return st;
@@ -277,6 +282,7 @@ slp::GemmArgs gemm_args(L* h, int mode, int e_begin, int e_end, int T) {
   g.E = h->E;
   g.T = T;
   g.n_stage = h->n_stage;
+  g.n_slots = 1 + h->n_stage;
   g.a_q = mode == 0 ? h->d_xq : h->d_hq;
   g.a_s = mode == 0 ? h->d_xs : h->d_hs;
   g.a_s_stride = mode == 0 ? h->xs_stride : h->hs_stride;
@@ -356,14 +362,32 @@ slp_status launch_experts(L* h, cudaStream_t s, int e_begin, int e_end, int T, i
   return SLP_OK;
 }
 
-slp_status copy_expert(L* h, int e) {
-  const size_t IH = static_cast<size_t>(h->I) * h->H;
-  uint8_t* slot = h->d_pool + static_cast<size_t>(1 + e % h->n_stage) * h->slot_bytes;
-  CU_TRY(cudaMemcpyAsync(slot, h->gate_q[e], IH, cudaMemcpyHostToDevice, h->copy_stream));
-  CU_TRY(cudaMemcpyAsync(slot + IH, h->up_q[e], IH, cudaMemcpyHostToDevice, h->copy_stream));
-  CU_TRY(cudaMemcpyAsync(slot + 2 * IH, h->down_q[e], IH, cudaMemcpyHostToDevice, h->copy_stream));
-  h->stats.bytes_copied += static_cast<int64_t>(3 * IH);
-  h->stats.experts_copied += 1;
+// Enqueues the host -> HBM copies of the wanted experts of [e0, e1) on the copy stream.  Runs of
+// experts whose host matrices AND ring slots are both consecutive are merged into one copy per kind.
+slp_status copy_experts(L* h, int e0, int e1, const int32_t* counts /* NULL = all wanted */) {
+  const size_t IH = static_cast<size_t>(h->I) * h->H, S = static_cast<size_t>(1 + h->n_stage);
+  const std::vector<const uint8_t*>* src[3] = {&h->gate_q, &h->up_q, &h->down_q};
+  auto wanted = [&](int e) { return !counts || counts[e] > 0; };
+  for (int kind = 0; kind < 3; ++kind) {
+    const std::vector<const uint8_t*>& p = *src[kind];
+    uint8_t* region = h->d_pool + static_cast<size_t>(kind) * S * IH;
+    for (int e = e0; e < e1;) {
+      if (!wanted(e)) { ++e; continue; }
+      int n = 1;  // experts e .. e + n - 1 in one copy
+      while (e + n < e1 && wanted(e + n) && p[e + n] == p[e] + static_cast<size_t>(n) * IH &&
+             (e + n) % h->n_stage == e % h->n_stage + n)
+        ++n;
+      CU_TRY(cudaMemcpyAsync(region + static_cast<size_t>(1 + e % h->n_stage) * IH, p[e], static_cast<size_t>(n) * IH,
+                             cudaMemcpyHostToDevice, h->copy_stream));
+      h->stats.h2d_copies += 1;
+      e += n;
+    }
+  }
+  for (int e = e0; e < e1; ++e)
+    if (wanted(e)) {
+      h->stats.bytes_copied += static_cast<int64_t>(3 * IH);
+      h->stats.experts_copied += 1;
+    }
   return SLP_OK;
 }
 
@@ -484,12 +508,10 @@ slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t
         CU_TRY(cudaEventRecord(h->ev_copy0, h->copy_stream));
         first_copy = false;
       }
-      for (int e = e0; e < e1; ++e) {
-        if (skip && h->h_counts[e] == 0) {
-          h->stats.experts_skipped += 1;
-          continue;
-        }
-        slp_status st = copy_expert(h, e);
+      for (int e = e0; e < e1; ++e)
+        if (skip && h->h_counts[e] == 0) h->stats.experts_skipped += 1;
+      {
+        slp_status st = copy_experts(h, e0, e1, skip ? h->h_counts : nullptr);
         if (st != SLP_OK) return st;
       }
       CU_TRY(cudaEventRecord(h->ev_ready[r], h->copy_stream));  // ON
@@ -727,10 +749,8 @@ slp_status slp_moe_set_residency(slp_moe_layer* h, slp_residency r) {
     st = alloc_pool(h, h->E, h->E);
     if (st != SLP_OK) return st;
     h->stats = slp_moe_stats{};
-    for (int e = 0; e < h->E; ++e) {
-      st = copy_expert(h, e);
-      if (st != SLP_OK) return st;
-    }
+    st = copy_experts(h, 0, h->E, nullptr);
+    if (st != SLP_OK) return st;
     CU_TRY(cudaStreamSynchronize(h->copy_stream));
   } else {
     int n_stage = h->cfg.staging_slots == 0 ? h->E : std::min(h->cfg.staging_slots, h->E);
