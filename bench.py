@@ -139,7 +139,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-resident-extra", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
-    ap.add_argument("--gemm-impl", type=int, default=0)
+    ap.add_argument("--triage", default=None, help="SLP_TRIAGE value for A/B runs (e.g. gemm=pair); not a product option")
     ap.add_argument("--staging-slots", type=int, default=0)
     ap.add_argument("--experts-per-launch", type=int, default=0)
     args = ap.parse_args()
@@ -201,7 +201,7 @@ def main():
     hidden = inputs.make_hidden(cfg, device=dev, first_chunk=sharding.weak_scaling_first_chunk(cfg.T, rank))  # each rank its own tokens
     t_gen = time.perf_counter() - t_gen
     layer = SlpMoeLayer(cfg, W, device=local_rank, staging_slots=args.staging_slots,
-                        experts_per_launch=args.experts_per_launch, gemm_impl=args.gemm_impl)
+                        experts_per_launch=args.experts_per_launch, triage=args.triage)
     layer.set_residency(mode)
     out = torch.empty_like(hidden)
     stream = torch.cuda.current_stream()
@@ -310,7 +310,7 @@ def main():
         try:
             layer.close()
             cfg2 = inputs.CONFIGS[2]
-            big = SlpMoeLayer(cfg2, W, device=local_rank, gemm_impl=args.gemm_impl)
+            big = SlpMoeLayer(cfg2, W, device=local_rank, triage=args.triage)
             big.set_residency("resident")
             h2 = inputs.make_hidden(cfg2, device=dev)
             o2 = torch.empty_like(h2)

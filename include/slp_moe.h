@@ -78,16 +78,6 @@ typedef struct {
                                  prefill).  0: paper-faithful fixed order, every expert copied. */
   int32_t require_pinned;     /* 1: create fails with SLP_ERR_NOT_PINNED if a weight buffer is
                                  pageable.  0: create pins it with cudaHostRegister. */
-  int32_t gemm_impl;          /* 0: tcgen05/TMEM/TMA grouped GEMM, one CTA per 128 x 256 tile, tiles handed out
-                                    through a global counter (the product path).
-                                 1: plain CUDA-core grouped GEMM kept for bring-up and for triaging the
-                                    tensor-core kernels; same kernels around it.
-                                 2: the cta_group::2 variant of the tcgen05 kernel (clusters of two CTAs).
-                                 3: as 0 with a static round-robin tile order (reads the operands from DRAM
-                                    ~2.7 times instead of once; kept for A/B). */
-  int32_t router_impl;        /* 0: router logits on the tensor cores (bf16 hi+lo split of the fp32
-                                 router weights, fp32 accumulate).  1: plain fp32 FMA kernel
-                                 (bring-up / triage). */
 } slp_moe_cfg;
 
 /* Host weight pointers.  Borrowed for the lifetime of the handle; the host copy stays
@@ -183,10 +173,21 @@ slp_status slp_moe_set_residency(slp_moe_layer* h, slp_residency r);
 /* out[t,:] = sum_j w[t,j] * FFN_{idx[t,j]}(hidden[t,:]) + FFN_shared(hidden[t,:]), bf16, no residual.
  *  hidden_bf16: dev [T, H] bf16, read only.  out_bf16: dev [T, H] bf16, fully overwritten; must
  *  not alias hidden.  T in 0..max_tokens (T == 0 returns SLP_OK and touches nothing).
- *  cuda_stream: a cudaStream_t (0 = legacy default stream).  Asynchronous: all work is ordered
- *  after prior work on cuda_stream and `out` is valid for later work on it.  The library's copy
- *  stream is joined to cuda_stream by events.  One call in flight per handle: a second call
- *  before the first has finished on the device returns SLP_ERR_BUSY.
+ *  cuda_stream: a cudaStream_t (0 = legacy default stream).  Asynchronous: every kernel of the call is
+ *  ordered after prior work on cuda_stream and `out` is valid for later work on it.
+ *  Copy stream (streamed mode): the host -> HBM expert copies run on the library's own copy stream.  They
+ *  wait only for the ring slot they overwrite to be free (the OFF event of the launch that last used it,
+ *  PAPER.md:138), NOT for prior work on cuda_stream: the weights do not depend on anything the caller
+ *  computes, so the first copies of a call start as soon as the call is enqueued, and across back-to-back
+ *  calls on one stream the next call's copies overlap the current call's last GEMMs (cross-call prefetch,
+ *  the single-layer form of the paper's "load the next module while this one executes").  The kernels that
+ *  consume a slot wait for its ON event, and the call's last record on cuda_stream follows all of them, so
+ *  `out` ordering is unaffected.  The host weight buffers must not change while a handle borrows them.
+ *  Calls in flight: calls on ONE stream may be enqueued back to back without waiting (they serialise on the
+ *  stream and share the workspace safely); slp_moe_get_stats then describes the most recent call.  A call
+ *  on a DIFFERENT stream while the previous call has not finished on the device returns SLP_ERR_BUSY (the
+ *  workspace is per handle).  If the previous call has finished and one of its kernels hit the in-kernel
+ *  watchdog, this call returns SLP_ERR_KERNEL_TIMEOUT and enqueues nothing.
  *  With skip_empty_experts == 1 the call synchronises cuda_stream once internally. */
 slp_status slp_moe_prefill(slp_moe_layer* h, const void* hidden_bf16, int32_t T, void* out_bf16, void* cuda_stream);
 
@@ -206,6 +207,9 @@ slp_status slp_moe_debug_routing(slp_moe_layer* h, int32_t* idx /*[T,k]*/, float
 slp_status slp_moe_debug_quant_hidden(slp_moe_layer* h, uint8_t* xq /*[T,H]*/, float* xs /*[T,H/128]*/);
 /* Copies min(bytes, size of the buffer for the last call) bytes; *written gets that size. */
 slp_status slp_moe_debug_buffer(slp_moe_layer* h, int32_t which, void* host_dst, size_t bytes, size_t* written);
+/* Copies `bytes` bytes starting `offset` bytes into the same buffer (full-size parity tests read single
+ * experts' rows of hq / hs / Y instead of gigabytes).  INVALID_ARG if the range leaves the buffer. */
+slp_status slp_moe_debug_buffer_range(slp_moe_layer* h, int32_t which, size_t offset, size_t bytes, void* host_dst);
 slp_status slp_moe_get_stats(slp_moe_layer* h, slp_moe_stats* stats);
 
 /* Measures pinned host -> device bandwidth on `device` with back-to-back cudaMemcpyAsync of

@@ -15,7 +15,7 @@ EXPORTED_SYMBOLS = [
     "slp_moe_layer_create", "slp_moe_set_residency", "slp_moe_prefill", "slp_moe_prefill_host",
     "slp_moe_layer_destroy", "slp_last_error", "slp_moe_debug_routing",
     "slp_moe_debug_quant_hidden", "slp_moe_debug_buffer", "slp_moe_get_stats",
-    "slp_measure_h2d", "slp_version", "slp_moe_query_plan",
+    "slp_measure_h2d", "slp_version", "slp_moe_query_plan", "slp_moe_debug_buffer_range",
 ]
 
 SLP_STREAMED, SLP_RESIDENT = 0, 1
@@ -37,8 +37,7 @@ class _Cfg(C.Structure):
                 ("scoring", C.c_int32), ("norm_topk", C.c_int32), ("routed_scale", C.c_float),
                 ("max_tokens", C.c_int32), ("staging_slots", C.c_int32),
                 ("experts_per_launch", C.c_int32), ("skip_empty_experts", C.c_int32),
-                ("require_pinned", C.c_int32), ("gemm_impl", C.c_int32),
-                ("router_impl", C.c_int32)]
+                ("require_pinned", C.c_int32)]
 
 
 class _HostWeights(C.Structure):
@@ -88,6 +87,7 @@ def lib():
         L.slp_moe_debug_routing.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.slp_moe_debug_quant_hidden.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.slp_moe_debug_buffer.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_size_t, C.POINTER(C.c_size_t)]
+        L.slp_moe_debug_buffer_range.argtypes = [C.c_void_p, C.c_int32, C.c_size_t, C.c_size_t, C.c_void_p]
         L.slp_moe_get_stats.argtypes = [C.c_void_p, C.POINTER(Stats)]
         L.slp_measure_h2d.argtypes = [C.c_int32, C.c_size_t, C.c_size_t, C.c_int32, C.POINTER(C.c_double)]
         for name in EXPORTED_SYMBOLS:
@@ -130,15 +130,14 @@ class Plan(C.Structure):
 
 
 def _make_cfg(cfg, *, max_tokens=None, device=0, staging_slots=0, experts_per_launch=0, skip_empty_experts=False,
-              require_pinned=False, gemm_impl=0, router_impl=0):
+              require_pinned=False):
     return _Cfg(struct_size=C.sizeof(_Cfg), device=device, hidden=cfg.H, n_experts=cfg.E,
                 top_k=cfg.k, n_group=cfg.G, topk_group=cfg.Gk, moe_intermediate=cfg.I,
                 n_shared=cfg.n_shared, shared_intermediate=cfg.I if cfg.n_shared else 0,
                 scoring=SCORING[cfg.scoring], norm_topk=int(cfg.norm_topk),
                 routed_scale=cfg.routed_scale, max_tokens=max_tokens or cfg.T,
                 staging_slots=staging_slots, experts_per_launch=experts_per_launch,
-                skip_empty_experts=int(skip_empty_experts), require_pinned=int(require_pinned),
-                gemm_impl=gemm_impl, router_impl=router_impl)
+                skip_empty_experts=int(skip_empty_experts), require_pinned=int(require_pinned))
 
 
 def query_plan(cfg, **kw):
@@ -155,14 +154,16 @@ class SlpMoeLayer:
     tensors, kept alive by this object because the library borrows the memory)."""
 
     def __init__(self, cfg, weights, *, max_tokens=None, device=0, staging_slots=0,
-                 experts_per_launch=0, skip_empty_experts=False, require_pinned=False, gemm_impl=0, router_impl=0):
+                 experts_per_launch=0, skip_empty_experts=False, require_pinned=False, triage=None):
+        """`triage`: value for the library's SLP_TRIAGE environment switch during create (e.g.
+        "gemm=simt", "gemm=pair,router=fp32"); bring-up / bisection only, not part of the ABI."""
         self._h = C.c_void_p()
         self.cfg = cfg
         self.weights = weights
         self.max_tokens = max_tokens or cfg.T
         c = _make_cfg(cfg, max_tokens=self.max_tokens, device=device, staging_slots=staging_slots,
                       experts_per_launch=experts_per_launch, skip_empty_experts=skip_empty_experts,
-                      require_pinned=require_pinned, gemm_impl=gemm_impl, router_impl=router_impl)
+                      require_pinned=require_pinned)
         w = weights
         self._arrays = {k: _ptr_array(w[k]) for k in ("gate_q", "gate_s", "up_q", "up_s", "down_q", "down_s")}
 
@@ -175,7 +176,17 @@ class SlpMoeLayer:
                           shared_down_q=p(w["shared_down_q"]), shared_down_s=p(w["shared_down_s"]))
         for k, arr in self._arrays.items():
             setattr(hw, k, C.cast(arr, C.POINTER(C.c_void_p)))
-        _check(lib().slp_moe_layer_create(C.byref(c), C.byref(hw), C.byref(self._h)))
+        saved = os.environ.get("SLP_TRIAGE")
+        if triage is not None:
+            os.environ["SLP_TRIAGE"] = triage
+        try:
+            _check(lib().slp_moe_layer_create(C.byref(c), C.byref(hw), C.byref(self._h)))
+        finally:
+            if triage is not None:
+                if saved is None:
+                    os.environ.pop("SLP_TRIAGE", None)
+                else:
+                    os.environ["SLP_TRIAGE"] = saved
 
     # -- the C-ABI calls ------------------------------------------------------------------
     def set_residency(self, mode):
@@ -220,6 +231,15 @@ class SlpMoeLayer:
         buf = np.empty(size.value, np.uint8)
         _check(lib().slp_moe_debug_buffer(self._h, BUF[name], buf.ctypes.data, size.value, C.byref(size)))
         return buf.view(dtype)
+
+    def debug_rows(self, name, dtype, row0, nrows, row_elems):
+        """Rows [row0, row0 + nrows) of a row-major debug buffer whose rows hold `row_elems` elements of
+        `dtype` (slp_moe_debug_buffer_range): single experts' hq / hs / Y rows of a full-size layer."""
+        import numpy as np
+        item = np.dtype(dtype).itemsize
+        out = np.empty((nrows, row_elems), dtype)
+        _check(lib().slp_moe_debug_buffer_range(self._h, BUF[name], row0 * row_elems * item, out.nbytes, out.ctypes.data))
+        return out
 
     def stats(self):
         st = Stats(struct_size=C.sizeof(Stats))

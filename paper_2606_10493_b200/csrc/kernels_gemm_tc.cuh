@@ -3,7 +3,7 @@
 // One persistent CTA per SM works through the (128-row tile, N tile) work items of the experts of the
 // launch (one 16-byte record per tile, written by permute_scan_kernel); an otherwise idle warp takes the
 // items from a global counter, so all CTAs stay within ~gridDim consecutive items and share operands
-// through L2 (cfg.gemm_impl = 3: static round-robin instead).  Per
+// through L2 (SLP_TRIAGE gemm=static: static round-robin instead).  Per
 // 128-deep K block the tensor core writes a fresh 128 x 256 fp32 partial into one of two TMEM
 // buffers; the promotion warps pull it out with tcgen05.ld and add it into fp32 register accumulators
 // with one FMA per element (issued as FFMA2 pairs), scaled by  xs[row, kb] * ws[n-block, kb]
@@ -21,7 +21,7 @@
 //               of half w / 4; 128 fp32 accumulators per thread; the TMEM buffer is handed back as
 //               soon as the last tcgen05.ld has landed, before the last FMAs
 //
-// kPair (cfg.gemm_impl = 2): a cluster of two CTAs issues ONE cta_group::2 MMA with M = 256 (two
+// kPair (SLP_TRIAGE gemm=pair): a cluster of two CTAs issues ONE cta_group::2 MMA with M = 256 (two
 //   128-row tiles of the same expert) x N = 256; each CTA stages its own A tile and half of the B tile
 //   (TMA loads of both CTAs complete on the leader's mbarrier, commits are multicast to both CTAs, the
 //   peer's promotion warps release TMEM on the leader's barrier).  It moves a third less operand data
@@ -197,7 +197,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
   };
 
   // Next work item of this CTA after `w` (its i-th), or -1.  Static order: w + gridDim.  kDyn (one-CTA
-  // kernel, the default; cfg.gemm_impl = 3 selects the static order): items come from a global counter through a small shared-memory ring fed by an idle warp, so
+  // kernel, the default; SLP_TRIAGE gemm=static selects the static order): items come from a global counter through a small shared-memory ring fed by an idle warp, so
   // all CTAs stay inside a window of ~gridDim consecutive items and the B tiles they share stay in L2
   // (profiles/r1_sched_ab.md).  Which CTA computes a tile does not change its result.
   auto next_item = [&](int w, int i, bool whole_warp) -> int {
@@ -226,7 +226,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
     if (ptx::elect_one()) {
       int stage = 0;
       uint32_t phase = 0;
-      Tile nx = fetch(min(w_first, max(total - 1, 0)));
+      Tile nx{0, 0, 0, 0};
+      if (w_first < total) nx = fetch(w_first);  // idle CTAs (and launches without any tile) read no record
       int w = w_first < total ? w_first : -1;
       for (int i = 0; w >= 0; ++i) {
         const Tile cur = nx;
@@ -345,8 +346,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
       w0_nxt = lane < num_kb ? ws0[lane] : 0.f;
       w1_nxt = (kMode == 0 && lane < num_kb) ? ws1[lane] : 0.f;
     };
-    Tile nx = fetch(min(w_first, max(total - 1, 0)));
-    if (w_first < total) open_tile(nx);
+    Tile nx{0, 0, 0, 0};
+    if (w_first < total) { nx = fetch(w_first); open_tile(nx); }
     int w = w_first < total ? w_first : -1;
     for (int i = 0; w >= 0; ++i, tile_parity ^= 1) {
       const Tile cur = nx;

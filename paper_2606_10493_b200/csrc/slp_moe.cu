@@ -11,6 +11,7 @@
 #include <algorithm>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <new>
@@ -105,6 +106,30 @@ inline int auto_epl(int n_stage, int E) {
 
 inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
 
+// Triage switches, read once per create from the environment variable SLP_TRIAGE (comma-separated tokens);
+// not part of the ABI.  They select bring-up / A-B variants of two kernels so a wrong result can be
+// bisected on a GPU box without rebuilding:
+//   gemm=simt    plain CUDA-core grouped GEMM (kernels_gemm_simt.cuh) instead of the tcgen05 kernels
+//   gemm=static  one-CTA tcgen05 kernel with the static round-robin tile order
+//   gemm=pair    the cta_group::2 variant of the tcgen05 kernel
+//   router=fp32  router logits as plain fp32 FMAs instead of the tensor-core hi/lo split
+enum GemmImpl { kGemmTc = 0, kGemmSimt = 1, kGemmPair = 2, kGemmStatic = 3 };
+struct Triage {
+  int gemm = kGemmTc;
+  int router_fp32 = 0;
+};
+inline Triage read_triage() {
+  Triage t;
+  const char* env = std::getenv("SLP_TRIAGE");
+  if (!env) return t;
+  const std::string v(env);
+  if (v.find("gemm=simt") != std::string::npos) t.gemm = kGemmSimt;
+  else if (v.find("gemm=static") != std::string::npos) t.gemm = kGemmStatic;
+  else if (v.find("gemm=pair") != std::string::npos) t.gemm = kGemmPair;
+  if (v.find("router=fp32") != std::string::npos) t.router_fp32 = 1;
+  return t;
+}
+
 // Shape / option validation shared by create and slp_moe_query_plan (no CUDA calls).  On success
 // *n_stage = expert slots of the streamed ring, *epl = experts per grouped-GEMM launch.
 slp_status validate_cfg(const slp_moe_cfg* cfg, int* n_stage_out, int* epl_out) {
@@ -119,8 +144,6 @@ slp_status validate_cfg(const slp_moe_cfg* cfg, int* n_stage_out, int* epl_out) 
     return fail(SLP_ERR_UNSUPPORTED_SHAPE, "n_shared must be 0 or 1 with shared_intermediate == moe_intermediate");
   if (cfg->scoring != SLP_SCORE_SIGMOID_BIAS && cfg->scoring != SLP_SCORE_SOFTMAX) return fail(SLP_ERR_INVALID_ARG, "unknown scoring %d", cfg->scoring);
   if (cfg->max_tokens <= 0) return fail(SLP_ERR_INVALID_ARG, "max_tokens must be positive");
-  if (cfg->gemm_impl < 0 || cfg->gemm_impl > 3) return fail(SLP_ERR_INVALID_ARG, "gemm_impl must be 0, 1, 2 or 3");
-  if (cfg->router_impl != 0 && cfg->router_impl != 1) return fail(SLP_ERR_INVALID_ARG, "router_impl must be 0 or 1");
   int n_stage = cfg->staging_slots == 0 ? E : cfg->staging_slots;
   if (n_stage < 2 && E >= 2) return fail(SLP_ERR_INVALID_ARG, "staging_slots must be 0 or 2..n_experts");
   n_stage = std::min(n_stage, E);
@@ -137,6 +160,7 @@ slp_status validate_cfg(const slp_moe_cfg* cfg, int* n_stage_out, int* epl_out) 
 
 struct slp_moe_layer {
   slp_moe_cfg cfg{};
+  Triage triage{};
   slp_moe_host_weights hw{};
   std::vector<const uint8_t*> gate_q, up_q, down_q;
   std::vector<void*> registered;  // host ranges pinned by create
@@ -176,6 +200,8 @@ struct slp_moe_layer {
   std::vector<char> free_recorded;
   cudaEvent_t ev_done = nullptr, ev_t[6] = {}, ev_copy0 = nullptr, ev_copy1 = nullptr;
   bool in_flight = false;
+  bool dead = false;               // the expert pool could not be restored after a failed residency switch
+  bool pool_needs_upload = false;  // resident pool was rebuilt after a failed switch: experts must be re-uploaded
   cudaStream_t last_stream = nullptr;
   int last_T = 0;
   slp_moe_stats stats{};
@@ -188,24 +214,34 @@ namespace {
 
 using L = slp_moe_layer;
 
+struct Pool {
+  uint8_t* d_pool = nullptr;
+  std::vector<cudaEvent_t> ev_ready, ev_free;
+  CUtensorMap tm_wgu{}, tm_wd{};
+};
+
+void release_pool(Pool* p) {
+  if (p->d_pool) cudaFree(p->d_pool);
+  p->d_pool = nullptr;
+  for (auto e : p->ev_ready) cudaEventDestroy(e);
+  for (auto e : p->ev_free) cudaEventDestroy(e);
+  p->ev_ready.clear();
+  p->ev_free.clear();
+}
+
 void free_pool(L* h) {
-  if (h->d_pool) cudaFree(h->d_pool);
+  Pool p;
+  p.d_pool = h->d_pool;
+  p.ev_ready.swap(h->ev_ready);
+  p.ev_free.swap(h->ev_free);
+  release_pool(&p);
   h->d_pool = nullptr;
-  for (auto e : h->ev_ready) cudaEventDestroy(e);
-  for (auto e : h->ev_free) cudaEventDestroy(e);
-  h->ev_ready.clear();
-  h->ev_free.clear();
   h->free_recorded.clear();
 }
 
-// (Re)allocates the expert pool with `n_stage` routed slots (+ slot 0 for the shared expert),
-// uploads the shared expert, rebuilds the weight tensor maps and the ring events.
-slp_status alloc_pool(L* h, int n_stage, int epl) {
-  free_pool(h);
-  h->n_stage = n_stage;
-  h->epl = epl;
+slp_status build_pool(L* h, int n_stage, int epl, Pool* p) {
   const size_t bytes = static_cast<size_t>(1 + n_stage) * h->slot_bytes;
-  CU_TRY(cudaMalloc(&h->d_pool, bytes));
+  CU_TRY(cudaMalloc(&p->d_pool, bytes));
   const size_t IH = static_cast<size_t>(h->I) * h->H;
   // Pool layout: [gate of all slots | up of all slots | down of all slots], slot 0 = shared expert.
   // Kind-major so that experts that are contiguous in host memory (stacked [E, I, H] tensors, the usual
@@ -213,37 +249,111 @@ slp_status alloc_pool(L* h, int n_stage, int epl) {
   // ~4 us gap between back-to-back 14.7 MB copies is 1.5 % of the link time (profiles/r1_h2d_chunks.md).
   const size_t S = static_cast<size_t>(1 + n_stage);
   if (h->cfg.n_shared) {
-    CU_TRY(cudaMemcpy(h->d_pool, h->hw.shared_gate_q, IH, cudaMemcpyHostToDevice));
-    CU_TRY(cudaMemcpy(h->d_pool + S * IH, h->hw.shared_up_q, IH, cudaMemcpyHostToDevice));
-    CU_TRY(cudaMemcpy(h->d_pool + 2 * S * IH, h->hw.shared_down_q, IH, cudaMemcpyHostToDevice));
+    CU_TRY(cudaMemcpy(p->d_pool, h->hw.shared_gate_q, IH, cudaMemcpyHostToDevice));
+    CU_TRY(cudaMemcpy(p->d_pool + S * IH, h->hw.shared_up_q, IH, cudaMemcpyHostToDevice));
+    CU_TRY(cudaMemcpy(p->d_pool + 2 * S * IH, h->hw.shared_down_q, IH, cudaMemcpyHostToDevice));
   } else {
-    for (int kind = 0; kind < 3; ++kind) CU_TRY(cudaMemset(h->d_pool + kind * S * IH, 0, IH));
+    for (int kind = 0; kind < 3; ++kind) CU_TRY(cudaMemset(p->d_pool + kind * S * IH, 0, IH));
   }
-  slp_status st = make_tmap_u8(&h->tm_wgu, h->d_pool, h->H, static_cast<uint64_t>(1 + n_stage) * 3 * h->I, slp::tc::kBoxRows);
+  slp_status st = make_tmap_u8(&p->tm_wgu, p->d_pool, h->H, static_cast<uint64_t>(1 + n_stage) * 3 * h->I, slp::tc::kBoxRows);
   if (st != SLP_OK) return st;
-  st = make_tmap_u8(&h->tm_wd, h->d_pool, h->I, static_cast<uint64_t>(1 + n_stage) * 3 * h->H, slp::tc::kBoxRows);
+  st = make_tmap_u8(&p->tm_wd, p->d_pool, h->I, static_cast<uint64_t>(1 + n_stage) * 3 * h->H, slp::tc::kBoxRows);
   if (st != SLP_OK) return st;
   const int n_groups = (n_stage + epl - 1) / epl;
-  h->ev_ready.resize(n_groups);
-  h->ev_free.resize(n_groups);
-  h->free_recorded.assign(n_groups, 0);
   for (int i = 0; i < n_groups; ++i) {
-    CU_TRY(cudaEventCreateWithFlags(&h->ev_ready[i], cudaEventDisableTiming));
-    CU_TRY(cudaEventCreateWithFlags(&h->ev_free[i], cudaEventDisableTiming));
+    cudaEvent_t a = nullptr, b = nullptr;
+    CU_TRY(cudaEventCreateWithFlags(&a, cudaEventDisableTiming));
+    p->ev_ready.push_back(a);
+    CU_TRY(cudaEventCreateWithFlags(&b, cudaEventDisableTiming));
+    p->ev_free.push_back(b);
   }
   return SLP_OK;
+}
+
+// (Re)allocates the expert pool with `n_stage` routed slots (+ slot 0 for the shared expert), uploads
+// the shared expert, rebuilds the weight tensor maps and the ring events.  `keep_old_until_built`:
+// the new pool is built next to the old one and swapped in only on success, so a failure (out of
+// memory on the way to resident mode) leaves the handle exactly as it was.  When both pools do not fit
+// side by side the old one is released first; if the new one then fails, the previous pool is rebuilt,
+// and only if that fails too is the handle marked dead (prefill then returns an error, never a launch
+// against a null pool).
+slp_status alloc_pool(L* h, int n_stage, int epl) {
+  Pool fresh;
+  slp_status st = build_pool(h, n_stage, epl, &fresh);
+  if (st != SLP_OK && h->d_pool) {
+    const std::string first_error = g_last_error;
+    release_pool(&fresh);
+    cudaGetLastError();
+    const int old_stage = h->n_stage, old_epl = h->epl;
+    free_pool(h);  // make room: the two pools did not fit side by side
+    st = build_pool(h, n_stage, epl, &fresh);
+    if (st != SLP_OK) {
+      release_pool(&fresh);
+      cudaGetLastError();
+      Pool back;
+      if (build_pool(h, old_stage, old_epl, &back) == SLP_OK) {
+        h->d_pool = back.d_pool;
+        h->ev_ready.swap(back.ev_ready);
+        h->ev_free.swap(back.ev_free);
+        h->tm_wgu = back.tm_wgu;
+        h->tm_wd = back.tm_wd;
+        h->free_recorded.assign(h->ev_ready.size(), 0);
+        h->pool_needs_upload = true;  // resident experts were lost with the old pool
+      } else {
+        release_pool(&back);
+        cudaGetLastError();
+        h->dead = true;
+      }
+      return fail(st, "expert pool of %d slots could not be allocated: %s", n_stage, first_error.c_str());
+    }
+  } else if (st != SLP_OK) {
+    release_pool(&fresh);
+    return st;
+  }
+  free_pool(h);
+  h->d_pool = fresh.d_pool;
+  h->ev_ready.swap(fresh.ev_ready);
+  h->ev_free.swap(fresh.ev_free);
+  h->tm_wgu = fresh.tm_wgu;
+  h->tm_wd = fresh.tm_wd;
+  h->free_recorded.assign(h->ev_ready.size(), 0);
+  h->n_stage = n_stage;
+  h->epl = epl;
+  return SLP_OK;
+}
+
+// true if [p, p + bytes) is page-locked host memory as far as the runtime can tell (first and last byte)
+bool range_is_pinned(const void* p, size_t bytes) {
+  const char* ends[2] = {static_cast<const char*>(p), static_cast<const char*>(p) + (bytes ? bytes - 1 : 0)};
+  for (const char* q : ends) {
+    cudaPointerAttributes attr{};
+    if (cudaPointerGetAttributes(&attr, q) != cudaSuccess || attr.type != cudaMemoryTypeHost) {
+      cudaGetLastError();
+      return false;
+    }
+  }
+  return true;
 }
 
 slp_status pin_range(L* h, const void* p, size_t bytes, const char* what) {
   cudaPointerAttributes attr{};
   cudaError_t e = cudaPointerGetAttributes(&attr, p);
-  if (e == cudaSuccess && (attr.type == cudaMemoryTypeHost || attr.type == cudaMemoryTypeManaged)) return SLP_OK;
+  if (e == cudaSuccess && attr.type == cudaMemoryTypeManaged)
+    return fail(SLP_ERR_NOT_PINNED, "%s is managed memory: the streaming engine needs page-locked host memory "
+                                    "(cudaMemcpyAsync from managed memory is staged and far below link rate)", what);
+  if (e == cudaSuccess && attr.type == cudaMemoryTypeDevice)
+    return fail(SLP_ERR_INVALID_ARG, "%s is a device pointer; host weights are expected", what);
   cudaGetLastError();
+  if (range_is_pinned(p, bytes)) return SLP_OK;
   if (h->cfg.require_pinned) return fail(SLP_ERR_NOT_PINNED, "%s is pageable host memory and require_pinned is set", what);
   e = cudaHostRegister(const_cast<void*>(p), bytes, cudaHostRegisterDefault);
   if (e == cudaErrorHostMemoryAlreadyRegistered) {
+    // part of the range (a page shared with a neighbouring tensor) was registered before: accept only if
+    // the whole range is page-locked now, otherwise the copies would silently fall back to staged transfers
     cudaGetLastError();
-    return SLP_OK;
+    if (range_is_pinned(p, bytes)) return SLP_OK;
+    return fail(SLP_ERR_NOT_PINNED, "%s overlaps an already registered range but is not page-locked end to end; "
+                                    "register the enclosing allocation once or pass pinned memory", what);
   }
   if (e != cudaSuccess) return fail(SLP_ERR_NOT_PINNED, "cudaHostRegister(%s, %zu bytes) failed: %s", what, bytes, cudaGetErrorString(e));
   h->registered.push_back(const_cast<void*>(p));
@@ -305,7 +415,7 @@ slp::GemmArgs gemm_args(L* h, int mode, int e_begin, int e_end, int T) {
 // Launches gate/up (+SwiGLU+requant) and down for experts [e_begin, e_end) on `s`.
 // `max_tiles` bounds the number of 128-row tiles in the range (host-side, no sync).
 slp_status launch_experts(L* h, cudaStream_t s, int e_begin, int e_end, int T, int max_tiles) {
-  if (h->cfg.gemm_impl == 1) {
+  if (h->triage.gemm == kGemmSimt) {
     slp::GemmArgs g0 = gemm_args(h, 0, e_begin, e_end, T), g1 = gemm_args(h, 1, e_begin, e_end, T);
     dim3 grid0(h->I / 128, max_tiles * 4), grid1(h->H / 128, max_tiles * 4);
     slp::gemm_simt_kernel<0><<<grid0, 256, 0, s>>>(g0);
@@ -314,9 +424,9 @@ slp_status launch_experts(L* h, cudaStream_t s, int e_begin, int e_end, int T, i
     slp::GemmArgs g0 = gemm_args(h, 0, e_begin, e_end, T), g1 = gemm_args(h, 1, e_begin, e_end, T);
     const int nt0 = h->I / 128, nt1 = (h->H + 255) / 256;
     cudaEvent_t* ev = (h->ev_k_used + 3 <= static_cast<int>(h->ev_k.size())) ? &h->ev_k[h->ev_k_used] : nullptr;
-    if (h->cfg.gemm_impl == 0) CU_TRY(cudaMemsetAsync(h->d_sched, 0, 2 * sizeof(int), s));  // work-item counters of the two launches below
+    if (h->triage.gemm == kGemmTc) CU_TRY(cudaMemsetAsync(h->d_sched, 0, 2 * sizeof(int), s));  // work-item counters of the two launches below
     if (ev) cudaEventRecord(ev[0], s);
-    if (h->cfg.gemm_impl == 2) {
+    if (h->triage.gemm == kGemmPair) {
       // CTA-pair kernel: clusters of two CTAs, one per SM; a work item is a pair of 128-row tiles
       namespace tc = slp::tc;
       const int n_cl = h->num_sms / 2;
@@ -341,7 +451,7 @@ slp_status launch_experts(L* h, cudaStream_t s, int e_begin, int e_end, int T, i
       const int grid0 = std::max(1, std::min(h->num_sms, max_tiles * nt0));
       const int grid1 = std::max(1, std::min(h->num_sms, max_tiles * nt1));
       namespace tc = slp::tc;
-      if (h->cfg.gemm_impl == 0) {  // dynamic tile distribution (the product path); 3 = static round-robin
+      if (h->triage.gemm == kGemmTc) {  // dynamic tile distribution (the product path); 3 = static round-robin
         tc::gemm_tc_kernel<0, false, true><<<grid0, tc::kThreads, tc::Cfg<0, false>::kSmemBytes, s>>>(h->tm_xq, h->tm_wgu, h->tm_y, g0);
         if (ev) cudaEventRecord(ev[1], s);
         tc::gemm_tc_kernel<1, false, true><<<grid1, tc::kThreads, tc::Cfg<1, false>::kSmemBytes, s>>>(h->tm_hq, h->tm_wd, h->tm_y, g1);
@@ -406,7 +516,7 @@ slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t
   CU_TRY(cudaEventRecord(h->ev_t[0], s));
   // ---- a1 router ----
   {
-    if (h->cfg.router_impl == 1) {
+    if (h->triage.router_fp32) {
       dim3 grid((T + 63) / 64, (E + 63) / 64);
       slp::router_logits_kernel<<<grid, 256, 0, s>>>(static_cast<const uint16_t*>(hidden), h->d_router_w, h->d_logits, T, H, E);
     } else {
@@ -577,6 +687,7 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
   L* h = new (std::nothrow) L();
   if (!h) return fail(SLP_ERR_OOM, "out of host memory");
   h->cfg = *cfg;
+  h->triage = read_triage();
   h->hw = *w;
   h->H = H; h->E = E; h->k = k; h->I = I; h->Tm = cfg->max_tokens;
   h->kbH = H / 128; h->kbI = I / 128;
@@ -613,12 +724,23 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
 
   // pin (or check) the streamed weights
   const size_t IH = static_cast<size_t>(I) * H;
-  for (int e = 0; e < E; ++e) {
+  for (int e = 0; e < E; ++e)
     if (!h->gate_q[e] || !h->up_q[e] || !h->down_q[e] || !w->gate_s[e] || !w->up_s[e] || !w->down_s[e])
       return bail(fail(SLP_ERR_INVALID_ARG, "NULL weight pointer for expert %d", e));
-    TRY_OR_BAIL(pin_range(h, h->gate_q[e], IH, "gate_q"));
-    TRY_OR_BAIL(pin_range(h, h->up_q[e], IH, "up_q"));
-    TRY_OR_BAIL(pin_range(h, h->down_q[e], IH, "down_q"));
+  {
+    // Experts stacked in one [E, I, H] host tensor are checked / registered as ONE range per run: adjacent
+    // matrices of a pageable allocation share a page, which cudaHostRegister refuses matrix by matrix.
+    const std::vector<const uint8_t*>* kinds[3] = {&h->gate_q, &h->up_q, &h->down_q};
+    const char* names[3] = {"gate_q", "up_q", "down_q"};
+    for (int kind = 0; kind < 3; ++kind) {
+      const std::vector<const uint8_t*>& p = *kinds[kind];
+      for (int e = 0; e < E;) {
+        int n = 1;
+        while (e + n < E && p[e + n] == p[e] + static_cast<size_t>(n) * IH) ++n;
+        TRY_OR_BAIL(pin_range(h, p[e], static_cast<size_t>(n) * IH, names[kind]));
+        e += n;
+      }
+    }
   }
 
   CU_OR_BAIL(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
@@ -685,6 +807,9 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
   CU_OR_BAIL(cudaMalloc(&h->d_sched, 2 * sizeof(int)));
   CU_OR_BAIL(cudaMalloc(&h->d_err, sizeof(int)));
   CU_OR_BAIL(cudaMemset(h->d_err, 0, sizeof(int)));
+  CU_OR_BAIL(cudaMemset(h->d_tile_expert, 0, static_cast<size_t>(h->tiles_max) * sizeof(int32_t)));
+  CU_OR_BAIL(cudaMemset(h->d_tile_info, 0, static_cast<size_t>(h->tiles_max) * sizeof(int4)));
+  CU_OR_BAIL(cudaMemset(h->d_pair_expert, 0, static_cast<size_t>(h->tiles_max) * sizeof(int32_t)));
   // padding rows are read by the tensor cores (their outputs are discarded): keep them finite
   CU_OR_BAIL(cudaMemset(h->d_xq, 0, rows * H));
   CU_OR_BAIL(cudaMemset(h->d_hq, 0, rows * I));
@@ -744,20 +869,34 @@ slp_status slp_moe_set_residency(slp_moe_layer* h, slp_residency r) {
   slp_status st = wait_idle(h);
   if (st != SLP_OK) return st;
   CU_TRY(cudaDeviceSynchronize());
-  if (static_cast<int>(r) == h->residency) return SLP_OK;
+  if (h->dead) return fail(SLP_ERR_OOM, "handle lost its expert pool in an earlier failed residency switch; destroy it");
+  auto upload_all = [&]() -> slp_status {
+    h->stats = slp_moe_stats{};
+    slp_status u = copy_experts(h, 0, h->E, nullptr);
+    if (u != SLP_OK) return u;
+    CU_TRY(cudaStreamSynchronize(h->copy_stream));
+    h->pool_needs_upload = false;
+    return SLP_OK;
+  };
+  if (static_cast<int>(r) == h->residency) {
+    if (r == SLP_RESIDENT && h->pool_needs_upload) return upload_all();
+    return SLP_OK;
+  }
   if (r == SLP_RESIDENT) {
     st = alloc_pool(h, h->E, h->E);
+    if (st != SLP_OK) return st;   // the handle is unchanged (still streamed) unless it reports itself dead
+    st = upload_all();
     if (st != SLP_OK) return st;
-    h->stats = slp_moe_stats{};
-    st = copy_experts(h, 0, h->E, nullptr);
-    if (st != SLP_OK) return st;
-    CU_TRY(cudaStreamSynchronize(h->copy_stream));
   } else {
     int n_stage = h->cfg.staging_slots == 0 ? h->E : std::min(h->cfg.staging_slots, h->E);
     int epl = h->cfg.experts_per_launch;
     if (epl == 0) epl = auto_epl(n_stage, h->E);
     st = alloc_pool(h, n_stage, epl);
-    if (st != SLP_OK) return st;
+    if (st != SLP_OK) {
+      // still resident; if the pool had to be rebuilt on the way back its experts are uploaded again
+      if (!h->dead && h->pool_needs_upload) upload_all();
+      return st;
+    }
   }
   h->residency = r;
   return SLP_OK;
@@ -771,10 +910,13 @@ slp_status slp_moe_prefill(slp_moe_layer* h, const void* hidden_bf16, int32_t T,
   if (hidden_bf16 == out_bf16) return fail(SLP_ERR_INVALID_ARG, "out must not alias hidden");
   CU_TRY(cudaSetDevice(h->cfg.device));
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  if (h->dead) return fail(SLP_ERR_OOM, "handle lost its expert pool in an earlier failed residency switch; destroy it");
   if (h->in_flight) {
     cudaError_t q = cudaEventQuery(h->ev_done);
     if (q == cudaSuccess) {
       h->in_flight = false;
+      slp_status ke = check_kernel_error(h);  // the previous call finished: did one of its kernels hit the watchdog?
+      if (ke != SLP_OK) return ke;
     } else if (q == cudaErrorNotReady) {
       if (s != h->last_stream) return fail(SLP_ERR_BUSY, "a call is still in flight on another stream");
     } else {
@@ -790,6 +932,7 @@ slp_status slp_moe_prefill_host(slp_moe_layer* h, const void* hidden_host, int32
   if (T == 0) return SLP_OK;
   if (!hidden_host || !out_host) return fail(SLP_ERR_INVALID_ARG, "NULL hidden/out");
   CU_TRY(cudaSetDevice(h->cfg.device));
+  if (h->dead) return fail(SLP_ERR_OOM, "handle lost its expert pool in an earlier failed residency switch; destroy it");
   slp_status st = wait_idle(h);
   if (st != SLP_OK) return st;
   const size_t bytes = static_cast<size_t>(h->Tm) * h->H * 2;
@@ -858,30 +1001,53 @@ slp_status slp_moe_debug_quant_hidden(slp_moe_layer* h, uint8_t* xq, float* xs) 
   return check_kernel_error(h);
 }
 
+namespace {
+// device address and size (for the last call) of a debug buffer
+slp_status locate_buffer(slp_moe_layer* h, int32_t which, const void** src, size_t* size) {
+  int32_t rs[1] = {0};  // row_start[E+1] = rows in use
+  CU_TRY(cudaMemcpy(rs, h->d_row_start + h->E + 1, sizeof(int32_t), cudaMemcpyDeviceToHost));
+  const size_t rows = static_cast<size_t>(rs[0]), T = h->last_T;
+  switch (which) {
+    case SLP_BUF_COUNTS: *src = h->d_counts; *size = h->E * sizeof(int32_t); break;
+    case SLP_BUF_ROW_START: *src = h->d_row_start; *size = (h->E + 1) * sizeof(int32_t); break;
+    case SLP_BUF_POS: *src = h->d_pos; *size = T * h->k * sizeof(int32_t); break;
+    case SLP_BUF_ROW_TOKEN: *src = h->d_row_token; *size = rows * sizeof(int32_t); break;
+    case SLP_BUF_HQ: *src = h->d_hq; *size = rows * h->I; break;
+    case SLP_BUF_HS: *src = h->d_hs; *size = rows * h->hs_stride * sizeof(float); break;
+    case SLP_BUF_Y: *src = h->d_y; *size = rows * h->H * sizeof(float); break;
+    case SLP_BUF_LOGITS: *src = h->d_logits; *size = T * h->E * sizeof(float); break;
+    default: return fail(SLP_ERR_INVALID_ARG, "unknown buffer id %d", which);
+  }
+  return SLP_OK;
+}
+}  // namespace
+
 slp_status slp_moe_debug_buffer(slp_moe_layer* h, int32_t which, void* dst, size_t bytes, size_t* written) {
   if (!h || !dst) return fail(SLP_ERR_INVALID_ARG, "NULL argument");
   CU_TRY(cudaSetDevice(h->cfg.device));
   slp_status st = wait_idle(h);
   if (st != SLP_OK) return st;
-  int32_t rs[2] = {0, 0};  // row_start[E+1] = rows in use
-  CU_TRY(cudaMemcpy(rs, h->d_row_start + h->E + 1, sizeof(int32_t), cudaMemcpyDeviceToHost));
-  const size_t rows = static_cast<size_t>(rs[0]), T = h->last_T;
   const void* src = nullptr;
   size_t size = 0;
-  switch (which) {
-    case SLP_BUF_COUNTS: src = h->d_counts; size = h->E * sizeof(int32_t); break;
-    case SLP_BUF_ROW_START: src = h->d_row_start; size = (h->E + 1) * sizeof(int32_t); break;
-    case SLP_BUF_POS: src = h->d_pos; size = T * h->k * sizeof(int32_t); break;
-    case SLP_BUF_ROW_TOKEN: src = h->d_row_token; size = rows * sizeof(int32_t); break;
-    case SLP_BUF_HQ: src = h->d_hq; size = rows * h->I; break;
-    case SLP_BUF_HS: src = h->d_hs; size = rows * h->hs_stride * sizeof(float); break;
-    case SLP_BUF_Y: src = h->d_y; size = rows * h->H * sizeof(float); break;
-    case SLP_BUF_LOGITS: src = h->d_logits; size = T * h->E * sizeof(float); break;
-    default: return fail(SLP_ERR_INVALID_ARG, "unknown buffer id %d", which);
-  }
+  st = locate_buffer(h, which, &src, &size);
+  if (st != SLP_OK) return st;
   const size_t n = std::min(size, bytes);
   if (n) CU_TRY(cudaMemcpy(dst, src, n, cudaMemcpyDeviceToHost));
   if (written) *written = size;
+  return check_kernel_error(h);
+}
+
+slp_status slp_moe_debug_buffer_range(slp_moe_layer* h, int32_t which, size_t offset, size_t bytes, void* dst) {
+  if (!h || !dst) return fail(SLP_ERR_INVALID_ARG, "NULL argument");
+  CU_TRY(cudaSetDevice(h->cfg.device));
+  slp_status st = wait_idle(h);
+  if (st != SLP_OK) return st;
+  const void* src = nullptr;
+  size_t size = 0;
+  st = locate_buffer(h, which, &src, &size);
+  if (st != SLP_OK) return st;
+  if (offset > size || bytes > size - offset) return fail(SLP_ERR_INVALID_ARG, "range [%zu, +%zu) leaves the buffer of %zu bytes", offset, bytes, size);
+  if (bytes) CU_TRY(cudaMemcpy(dst, static_cast<const char*>(src) + offset, bytes, cudaMemcpyDeviceToHost));
   return check_kernel_error(h);
 }
 

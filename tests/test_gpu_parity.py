@@ -83,7 +83,7 @@ def test_substeps_bit_exact(name):
     """Router indices (outside near-ties), quantised hidden bytes + scales (bit-exact, Q12) and
     the permutation (true inverse, expert-contiguous, ascending token id, 128-aligned ranges)."""
     cfg, W, hidden, ref = problem(name)
-    out, idx, w, counts, xq, xs, extra = run_gpu(cfg, W, hidden, "resident", gemm_impl=1)
+    out, idx, w, counts, xq, xs, extra = run_gpu(cfg, W, hidden, "resident", triage="gemm=simt")
     r = compare_routing(idx, w, ref["route"])
     assert r["passed"], r
     assert np.array_equal(xq, ref["xq"])
@@ -108,33 +108,33 @@ def test_substeps_bit_exact(name):
 @pytest.mark.parametrize("name", list(CASES))
 @pytest.mark.parametrize("mode", ["resident", "streamed"])
 def test_layer_parity_simt(name, mode):
-    check(name, mode, gemm_impl=1)
+    check(name, mode, triage="gemm=simt")
 
 
 @pytest.mark.parametrize("name", list(CASES))
 @pytest.mark.parametrize("mode", ["resident", "streamed"])
 def test_layer_parity_tcgen05(name, mode):
-    """gemm_impl 0: the product path (tcgen05 / TMEM / TMA, one CTA per 128 x 256 tile, dynamic tile order)."""
-    check(name, mode, gemm_impl=0)
+    """Default: the product path (tcgen05 / TMEM / TMA, one CTA per 128 x 256 tile, dynamic tile order)."""
+    check(name, mode, triage=None)
 
 
 @pytest.mark.parametrize("name", list(CASES))
 def test_layer_parity_tcgen05_cta_pair(name):
-    """gemm_impl 2: the cta_group::2 variant (clusters of two CTAs, pairs of 128-row tiles, dummy
+    """SLP_TRIAGE gemm=pair: the cta_group::2 variant (clusters of two CTAs, pairs of 128-row tiles, dummy
     tile for experts with an odd tile count)."""
-    check(name, "resident", gemm_impl=2)
+    check(name, "resident", triage="gemm=pair")
 
 
 @pytest.mark.parametrize("name", list(CASES))
 @pytest.mark.parametrize("mode", ["resident", "streamed"])
 def test_layer_parity_tcgen05_static_tiles(name, mode):
-    """gemm_impl 3: the one-CTA kernel with the static round-robin tile order."""
-    check(name, mode, gemm_impl=3)
+    """SLP_TRIAGE gemm=static: the one-CTA kernel with the static round-robin tile order."""
+    check(name, mode, triage="gemm=static")
 
 
 @pytest.mark.parametrize("T", [1, 127, 128, 129, 257])
-@pytest.mark.parametrize("gemm_impl", [0, 2, 3])
-def test_ragged_token_counts(T, gemm_impl):
+@pytest.mark.parametrize("triage", [None, "gemm=pair", "gemm=static"])
+def test_ragged_token_counts(T, triage):
     """Edge sizes: a single token, one row short of / exactly / one row past a 128-row tile."""
     cfg, W, hidden, _ = problem("mini_dsv3")
     sub = cfg.with_tokens(T)
@@ -142,7 +142,7 @@ def test_ragged_token_counts(T, gemm_impl):
     ref = moe_layer(inputs.hidden_as_bits(x), inputs.weights_as_numpy(W), top_k=cfg.k, n_group=cfg.G,
                     topk_group=cfg.Gk, scoring=cfg.scoring, norm_topk=cfg.norm_topk, routed_scale=cfg.routed_scale)
     for mode in ("resident", "streamed"):
-        out, idx, w, counts, *_ = run_gpu(sub, W, x, mode, gemm_impl=gemm_impl)
+        out, idx, w, counts, *_ = run_gpu(sub, W, x, mode, triage=triage)
         r = compare_routing(idx, w, ref["route"])
         o = compare_output(out, ref["out_f64"], r["members_equal"])
         assert r["passed"] and o["passed"], (T, mode, r, o)
@@ -150,8 +150,8 @@ def test_ragged_token_counts(T, gemm_impl):
 
 
 @pytest.mark.parametrize("name", ["mini_dsv3_ragged", "mini_zipf", "mini_softmax"])
-@pytest.mark.parametrize("gemm_impl", [0, 2])
-def test_expert_intermediates_against_oracle(name, gemm_impl):
+@pytest.mark.parametrize("triage", [None, "gemm=pair"])
+def test_expert_intermediates_against_oracle(name, triage):
     """a5-a7 row by row: the requantised SwiGLU output (hq, hs) and the per-row expert output Y of the
     tcgen05 kernels against the oracle's expert_ffn on the same quantised rows.  The e4m3 codes are an
     integer decision taken in fp32 on both sides (Q12); they may differ only where fp32-vs-fp64
@@ -161,7 +161,7 @@ def test_expert_intermediates_against_oracle(name, gemm_impl):
     from oracle import e4m3_decode as decode
     cfg, W, hidden, ref = problem(name)
     Wn = inputs.weights_as_numpy(W)
-    layer = SlpMoeLayer(cfg, W, device=0, gemm_impl=gemm_impl)
+    layer = SlpMoeLayer(cfg, W, device=0, triage=triage)
     try:
         layer.set_residency("resident")
         layer.prefill(hidden.cuda())
@@ -204,18 +204,18 @@ def test_expert_intermediates_against_oracle(name, gemm_impl):
         y_own = dequantize_rows_1x128(g_hq, g_hs) @ dequantize_weight_128x128(ws[4], ws[5]).T
         rms = np.sqrt((y_own ** 2).mean())
         assert np.abs(g_y - y_own).max() <= 2e-5 * rms + 1e-30, (e, np.abs(g_y - y_own).max() / rms)
-    print(name, gemm_impl, "codes", n_codes, "differ", n_flip)
+    print(name, triage, "codes", n_codes, "differ", n_flip)
     assert n_flip <= 1e-4 * n_codes   # observed: 4 of 718 848 (accumulation-order noise, SURVEY.md Q21 predicts ~2e-5)
 
 
 @pytest.mark.parametrize("name", list(CASES))
-@pytest.mark.parametrize("router_impl", [0, 1])
-def test_router_logits_error(name, router_impl):
+@pytest.mark.parametrize("triage", [None, "router=fp32"])
+def test_router_logits_error(name, triage):
     """Router logits (SLP_BUF_LOGITS) against the fp64 product.  The tensor-core router splits the
     fp32 weights into bf16 hi + lo (kernels_router_tc.cuh); its logit error must stay a decade
     below the 1e-4 near-tie allowance on the selection scores (|d sigmoid| <= |d logit| / 4)."""
     cfg, W, hidden, ref = problem(name)
-    layer = SlpMoeLayer(cfg, W, device=0, router_impl=router_impl)
+    layer = SlpMoeLayer(cfg, W, device=0, triage=triage)
     try:
         layer.set_residency("resident")
         layer.prefill(hidden.cuda())
@@ -227,7 +227,7 @@ def test_router_logits_error(name, router_impl):
     x = hidden.to(torch.float64).numpy()
     exact = x @ W["router_w"].to(torch.float64).numpy().T
     err = np.abs(logits - exact).max()
-    print(name, "router_impl", router_impl, "max |logit error|", err)
+    print(name, "triage", triage, "max |logit error|", err)
     assert err < 4e-5, err
     r = compare_routing(idx, w, ref["route"])
     assert r["passed"], r

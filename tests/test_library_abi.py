@@ -31,8 +31,8 @@ def test_exports_every_declared_symbol(built):
 
 
 def test_struct_sizes_match_header(built):
-    # 20 four-byte fields / 14 pointers / see header
-    assert ctypes.sizeof(binding._Cfg) == 20 * 4
+    # 18 four-byte fields / 14 pointers / see header
+    assert ctypes.sizeof(binding._Cfg) == 18 * 4
     assert ctypes.sizeof(binding._HostWeights) == 14 * 8
     assert ctypes.sizeof(binding.Stats) == 96  # 80 + sm_mhz_gateup, sm_mhz_down + h2d_copies, reserved
 
@@ -119,7 +119,7 @@ def test_query_plan_rejects_bad_options(built):
     from paper_2606_10493_b200 import inputs
     cfg = inputs.CONFIGS[1]
     for kw in (dict(staging_slots=1), dict(staging_slots=8, experts_per_launch=8), dict(staging_slots=9, experts_per_launch=2),
-               dict(gemm_impl=7), dict(router_impl=2), dict(max_tokens=-5)):
+               dict(max_tokens=-5)):
         with pytest.raises(binding.SlpError) as ei:
             binding.query_plan(cfg, **kw)
         assert ei.value.status == -1, kw
