@@ -152,8 +152,10 @@ typedef enum {
   SLP_BUF_ROW_TOKEN = 3,   /* int32 [rows] token id of each workspace row (-1 = padding) */
   SLP_BUF_HQ = 4,          /* uint8 [rows, I] requantised SwiGLU output */
   SLP_BUF_HS = 5,          /* float [rows, ceil4(I/128)] its scales */
-  SLP_BUF_Y = 6,           /* float [rows, H] per-row expert outputs */
-  SLP_BUF_LOGITS = 7       /* float [T, E] router logits */
+  SLP_BUF_Y = 6,           /* fp16 [rows, H] per-row expert outputs (before the routing weights), block-scaled:
+                              value = y16 * ys[row, column / 128] */
+  SLP_BUF_LOGITS = 7,      /* float [T, E] router logits */
+  SLP_BUF_YS = 8           /* float [rows, ceil4(H/128)] power-of-two scales of SLP_BUF_Y */
 } slp_debug_buffer_id;
 
 /* Create a layer.  Validates shapes, pins (or checks) the host weights, uploads the resident

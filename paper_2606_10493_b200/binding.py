@@ -20,7 +20,7 @@ EXPORTED_SYMBOLS = [
 
 SLP_STREAMED, SLP_RESIDENT = 0, 1
 SCORING = {"sigmoid_bias": 0, "softmax": 1}
-BUF = dict(counts=0, row_start=1, pos=2, row_token=3, hq=4, hs=5, y=6, logits=7)
+BUF = dict(counts=0, row_start=1, pos=2, row_token=3, hq=4, hs=5, y=6, logits=7, ys=8)
 
 
 class SlpError(RuntimeError):

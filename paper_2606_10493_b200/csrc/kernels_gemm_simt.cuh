@@ -37,7 +37,9 @@ struct GemmArgs {
   uint8_t* hq;                 // [rows, I]
   float* hs;                   // [rows, hs_stride]
   int hs_stride;
-  float* y;                    // [rows, H] fp32
+  uint16_t* y;                 // [rows, H] fp16 bit patterns, block-scaled: value = y * ys[row, column / 128]
+  float* ys;                   // [rows, ys_stride] power-of-two scales
+  int ys_stride;
   int* err;
   int* sched;                  // [2] work-item counters of the gate/up and down launches (zeroed before each launch pair)
   unsigned long long* clk;     // [4] {SM cycles, ns} of CTA 0 summed over gate/up launches, then over down launches
@@ -53,7 +55,7 @@ __device__ __forceinline__ float e4m3_to_float(uint8_t c) {
 
 __device__ __forceinline__ float silu_mul(float g, float u) { return g / (1.0f + expf(-g)) * u; }
 
-// kMode 0: gate/up + SwiGLU + requant -> hq, hs.  kMode 1: down -> y (fp32).
+// kMode 0: gate/up + SwiGLU + requant -> hq, hs.  kMode 1: down -> y (block-scaled fp16).
 // Block: 32 rows x 128 output channels, 256 threads; thread (ty, tx) owns rows ty*4..+3 and
 // channels tx, tx+32, tx+64, tx+96, so one warp covers all 128 channels of its 4 rows.
 template <int kMode>
@@ -149,9 +151,23 @@ __global__ void __launch_bounds__(256) gemm_simt_kernel(GemmArgs g) {
               static_cast<uint8_t>(__nv_cvt_float_to_fp8(__fdiv_rn(h[j], s), __NV_SATFINITE, __NV_E4M3));
         if (tx == 0) g.hs[row * g.hs_stride + nb] = s;
       }
-    } else if (r < nrows) {
+    } else {
+      // block-scaled fp16, same rule as the tensor-core kernel: amax of the row's 128 columns into [2^14, 2^15)
+      float amax = 0.f;
 #pragma unroll
-      for (int j = 0; j < 4; ++j) g.y[row * g.H + nb * BC + tx + 32 * j] = acc0[i][j];
+      for (int j = 0; j < 4; ++j) amax = fmaxf(amax, fabsf(acc0[i][j]));
+#pragma unroll
+      for (int off = 16; off > 0; off >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xFFFFFFFFu, amax, off));
+      const uint32_t eb = max(__float_as_uint(amax) >> 23, 14u);
+      const float mult = __uint_as_float((268u - eb) << 23);
+      if (r < nrows) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const __half hv = __float2half_rn(acc0[i][j] * mult);
+          g.y[row * g.H + nb * BC + tx + 32 * j] = *reinterpret_cast<const uint16_t*>(&hv);
+        }
+        if (tx == 0) g.ys[row * g.ys_stride + nb] = __uint_as_float((eb - 14u) << 23);
+      }
     }
   }
 }

@@ -34,9 +34,9 @@
 //   so each half holds the gate and up columns of the same 64 intermediate channels; epilogue
 //   h = silu(g) * u, row amax over the 128 channels (two halves, exchanged through smem),
 //   s = amax / 448, e4m3(h / s) -> hq, hs  ("SiLU(.) (.)"; Q14).
-// kMode 1 (down):   B = down rows n0..n0+255; epilogue: the fp32 Y tile leaves through a per-warp
-//   staging ring in shared memory and TMA stores (Y stays fp32 so that the only bf16 rounding of the
-//   layer is the final one in the combine).
+// kMode 1 (down):   B = down rows n0..n0+255; epilogue: the Y tile is stored as block-scaled fp16 (one
+//   power-of-two scale per row per 128 columns), staged whole in shared memory and leaves through TMA
+//   stores while the next tile's K loop runs.
 #pragma once
 #include <cstdint>
 #include <cuda.h>
@@ -62,15 +62,13 @@ constexpr int kSchedDepth = 4;  // work items the scheduler warp may run ahead o
 //                (16 KB + 16 KB per stage, 6 stages), which cuts the L2 -> SM operand traffic per MAC
 //                by a third (the 1-CTA kernel is L2-bandwidth bound, profiles/r1_gemm_baseline.md).
 template <int kMode, bool kPair> struct Cfg {
-  // The down kernel trades pipeline stages for a Y staging ring (two 32 x 32 fp32 boxes per warp): its
-  // tiles are only 16 K blocks long, so the epilogue (128 KB of fp32 per tile) must not wait long on
-  // TMA-store read-out.
+  // The down kernel trades one pipeline stage for a staging area that holds its whole fp16 Y tile
+  // (64 KB): its tiles are only 16 K blocks long, so the epilogue must not wait on TMA-store read-out.
   static constexpr int kStages = kPair ? (kMode == 1 ? 5 : 6) : (kMode == 1 ? 3 : 4);
   static constexpr int kABytes = BM * BK;
   static constexpr int kBBytes = (kPair ? BN / 2 : BN) * BK;
   static constexpr int kStageBytes = kABytes + kBBytes;
-  static constexpr int kYRing = 2;                                           // 4 KB boxes per warp in flight
-  static constexpr int kScratchBytes = kMode == 1 ? kEpiWarps * 4096 * kYRing : 32768;  // (mode 0: amax exchange only)
+  static constexpr int kScratchBytes = kMode == 1 ? kEpiWarps * 8192 : 32768;  // mode 1: the whole fp16 Y tile (two 4 KB boxes per warp); mode 0: amax exchange only
   static constexpr int kSmemBytes = kStages * kStageBytes + 1024 /*align*/ + 256 /*barriers*/ + kScratchBytes;
   static_assert(kSmemBytes <= 232448, "shared memory budget");
 };
@@ -124,7 +122,7 @@ __global__ void __launch_bounds__(kThreads, 1)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__ CUtensorMap tm_b,
                const __grid_constant__ CUtensorMap tm_y, GemmArgs g) {
   using C = Cfg<kMode, kPair>;
-  constexpr int kStages = C::kStages, kABytes = C::kABytes, kStageBytes = C::kStageBytes, kScratchBytes = C::kScratchBytes, kYRing = C::kYRing;
+  constexpr int kStages = C::kStages, kABytes = C::kABytes, kStageBytes = C::kStageBytes, kScratchBytes = C::kScratchBytes;
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   uint8_t* scratch = smem + kStages * kStageBytes;  // 1024-aligned: per-warp staging for the Y TMA stores / amax exchange
@@ -498,32 +496,45 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
           if (half == 0) g.hs[row * g.hs_stride + nt] = s;
         }
       } else {
-        // Y tile (fp32, so that the layer's only bf16 rounding is the one in the combine): each warp owns
-        // 32 rows x 128 columns and streams them out as four 32 x 32 boxes through a staging ring in shared memory (128-byte rows, 128B swizzle: conflict-free st.shared.v4, whole-line global writes) with TMA stores,
-        // so the global writes drain asynchronously while the warp starts the next tile's K loop.
-        // Rows past the expert's count are padding rows of the workspace; whole 32-row groups past it
-        // are skipped.
+        // Y tile, stored as block-scaled fp16: a thread owns one row x 128 columns, exactly one scale block.
+        // It takes the block's amax, scales by the power of two that puts amax into [2^14, 2^15) (exact),
+        // rounds to fp16 (10-bit mantissa: 2^-11 relative, an eighth of a bf16 step, with fp32's range
+        // through the per-block exponent; DESIGN.md 3.4 has the error budget) and writes the scale 2^e to
+        // ys[row, block].  Each warp's 32 rows x 128 columns = two 32 x 64 boxes (128-byte rows, 128B
+        // swizzle: conflict-free st.shared.v4, whole-line global writes).  The whole tile fits in the
+        // staging area, so the warp writes both boxes, hands them to TMA stores and starts the next tile's
+        // K loop without waiting for a free slot; the boxes of the previous tile were read out long ago
+        // (16 K blocks), the wait below is a formality.  Rows past the expert's count are padding rows of
+        // the workspace; whole 32-row groups past it are skipped.
         const int c0 = nt * BN + half * HN;
         if (c0 < g.H && q * 32 < nrows) {
-          const uint32_t stage_a = smem_a + kStages * kStageBytes + warp * (4096 * kYRing);  // kYRing x 4 KB per warp
-          const uint32_t sw = static_cast<uint32_t>(lane & 7);
+          float amax = 0.f;
 #pragma unroll
-          for (int c = 0; c < 4; ++c) {  // four boxes of 32 rows x 32 columns (128-byte rows, 128B swizzle)
-            const uint32_t dst = stage_a + (c % kYRing) * 4096;
-            if (lane == 0) ptx::bulk_wait_group_read<kYRing - 1>();  // the box that used this buffer kYRing boxes ago has been read out
-            __syncwarp();
+          for (int i = 0; i < 128; ++i) amax = fmaxf(amax, fabsf(acc[i]));
+          const uint32_t eb = max(__float_as_uint(amax) >> 23, 14u);          // biased exponent of amax (>= 0)
+          const float mult = __uint_as_float((268u - eb) << 23);                // 2^(14 - floor(log2 amax))
+          g.ys[row * g.ys_stride + (c0 >> 7)] = __uint_as_float((eb - 14u) << 23);  // 2^(floor(log2 amax) - 14)
+          const uint32_t stage_a = smem_a + kStages * kStageBytes + warp * 8192;
+          const uint32_t sw = static_cast<uint32_t>(lane & 7);
+          if (lane == 0) ptx::bulk_wait_group_read<0>();
+          __syncwarp();
+#pragma unroll
+          for (int c = 0; c < 2; ++c) {
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
-              const uint32_t a = dst + lane * 128 + ((static_cast<uint32_t>(j) ^ sw) << 4);
-              asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(a), "f"(acc[c * 32 + j * 4]), "f"(acc[c * 32 + j * 4 + 1]),
-                           "f"(acc[c * 32 + j * 4 + 2]), "f"(acc[c * 32 + j * 4 + 3]) : "memory");
+              const float* a8 = acc + c * 64 + j * 8;
+              const uint32_t dst = stage_a + c * 4096 + lane * 128 + ((static_cast<uint32_t>(j) ^ sw) << 4);
+              asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(dst), "r"(ptx::pack_f16x2(a8[0] * mult, a8[1] * mult)),
+                           "r"(ptx::pack_f16x2(a8[2] * mult, a8[3] * mult)), "r"(ptx::pack_f16x2(a8[4] * mult, a8[5] * mult)),
+                           "r"(ptx::pack_f16x2(a8[6] * mult, a8[7] * mult)) : "memory");
             }
-            ptx::fence_proxy_async_smem();
-            __syncwarp();
-            if (lane == 0) {
-              ptx::tma_store_2d_a(&tm_y, dst, c0 + c * 32, row0 + q * 32);
-              ptx::bulk_commit_group();
-            }
+          }
+          ptx::fence_proxy_async_smem();
+          __syncwarp();
+          if (lane == 0) {
+            ptx::tma_store_2d_a(&tm_y, stage_a, c0, row0 + q * 32);
+            ptx::tma_store_2d_a(&tm_y, stage_a + 4096, c0 + 64, row0 + q * 32);
+            ptx::bulk_commit_group();
           }
         }
       }

@@ -4,6 +4,7 @@
 #include <cstdint>
 #include <cuda_bf16.h>
 #include <cuda_fp8.h>
+#include <cuda_fp16.h>
 
 namespace slp {
 
@@ -503,12 +504,23 @@ __global__ void __launch_bounds__(256) quant_scatter_kernel(const uint16_t* __re
 
 // ---------------------------------------------------------------------------------------------
 // a9: weighted combine.  out[t] = sum_j w[t,j] * Y[pos[t,j]] (fixed j order, fp32 FMA) + Y[t]
-// (shared expert row, weight 1); Y is fp32 and the sum is rounded once to bf16.  Gather-based, no atomics.
+// (shared expert row, weight 1).  Y rows are block-scaled fp16 (y = y16 * ys[row, column / 128], ys a power
+// of two), the sum is fp32 and rounded once to bf16.  Gather-based, no atomics.
 // (PAPER.md:92 step 5 "A final weighted sum"; "router-weighted accumulation in F32".)
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) combine_kernel(const float* __restrict__ y, const int32_t* __restrict__ pos,
+__device__ __forceinline__ void fma_f16x8(float (&acc)[8], float s, const uint4& v) {
+  const uint32_t u[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&u[i]));
+    acc[2 * i] = fmaf(s, f.x, acc[2 * i]);
+    acc[2 * i + 1] = fmaf(s, f.y, acc[2 * i + 1]);
+  }
+}
+
+__global__ void __launch_bounds__(256) combine_kernel(const uint16_t* __restrict__ y, const float* __restrict__ ys, const int32_t* __restrict__ pos,
                                                       const float* __restrict__ w, __nv_bfloat16* __restrict__ out, int T, int H,
-                                                      int k, int has_shared) {
+                                                      int k, int has_shared, int ys_stride) {
   const int t = blockIdx.x;
   __shared__ int32_t s_row[32];
   __shared__ float s_w[32];
@@ -517,21 +529,23 @@ __global__ void __launch_bounds__(256) combine_kernel(const float* __restrict__ 
     s_w[threadIdx.x] = w[static_cast<size_t>(t) * k + threadIdx.x];
   }
   __syncthreads();
-  for (int c = threadIdx.x * 4; c < H; c += blockDim.x * 4) {
-    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+  for (int c = threadIdx.x * 8; c < H; c += blockDim.x * 8) {  // 8 channels = one 16-byte load per row
+    float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
     for (int j = 0; j < k; ++j) {
-      const float4 v = *reinterpret_cast<const float4*>(y + static_cast<size_t>(s_row[j]) * H + c);
-      const float wj = s_w[j];
-      acc.x = fmaf(wj, v.x, acc.x); acc.y = fmaf(wj, v.y, acc.y);
-      acc.z = fmaf(wj, v.z, acc.z); acc.w = fmaf(wj, v.w, acc.w);
+      const size_t row = s_row[j];
+      const uint4 v = *reinterpret_cast<const uint4*>(y + row * H + c);
+      fma_f16x8(acc, s_w[j] * ys[row * ys_stride + (c >> 7)], v);  // power-of-two block scale: the product is exact
     }
     if (has_shared) {
-      const float4 v = *reinterpret_cast<const float4*>(y + static_cast<size_t>(t) * H + c);
-      acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
+      const uint4 v = *reinterpret_cast<const uint4*>(y + static_cast<size_t>(t) * H + c);
+      fma_f16x8(acc, ys[static_cast<size_t>(t) * ys_stride + (c >> 7)], v);
     }
-    __nv_bfloat162 lo = __floats2bfloat162_rn(acc.x, acc.y), hi = __floats2bfloat162_rn(acc.z, acc.w);
-    *reinterpret_cast<uint2*>(out + static_cast<size_t>(t) * H + c) =
-        make_uint2(*reinterpret_cast<uint32_t*>(&lo), *reinterpret_cast<uint32_t*>(&hi));
+    uint4 o;
+    __nv_bfloat162 p0 = __floats2bfloat162_rn(acc[0], acc[1]), p1 = __floats2bfloat162_rn(acc[2], acc[3]);
+    __nv_bfloat162 p2 = __floats2bfloat162_rn(acc[4], acc[5]), p3 = __floats2bfloat162_rn(acc[6], acc[7]);
+    o.x = *reinterpret_cast<uint32_t*>(&p0); o.y = *reinterpret_cast<uint32_t*>(&p1);
+    o.z = *reinterpret_cast<uint32_t*>(&p2); o.w = *reinterpret_cast<uint32_t*>(&p3);
+    *reinterpret_cast<uint4*>(out + static_cast<size_t>(t) * H + c) = o;
   }
 }
 

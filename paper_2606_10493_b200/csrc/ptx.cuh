@@ -261,6 +261,12 @@ __device__ __forceinline__ void fma2(uint64_t& acc, uint32_t v0, uint32_t v1, ui
       "fma.rn.f32x2 %0, a, %3, %0;\n\t}"
       : "+l"(acc) : "r"(v0), "r"(v1), "l"(s2));
 }
+// (lo, hi) fp32 -> packed f16x2, round to nearest even; lo lands in the low half (the lower address)
+__device__ __forceinline__ uint32_t pack_f16x2(float lo, float hi) {
+  uint32_t r;
+  asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+  return r;
+}
 __device__ __forceinline__ void unpack2(uint64_t v, float& lo, float& hi) {
   asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
 }

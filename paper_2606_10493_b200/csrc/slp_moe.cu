@@ -78,15 +78,15 @@ slp_status make_tmap_u8(CUtensorMap* tm, void* base, uint64_t inner, uint64_t ro
   return SLP_OK;
 }
 
-// 2D fp32 tensor [rows, inner] for TMA stores of 32-column x 32-row boxes (128-byte rows, 128B swizzle).
-slp_status make_tmap_f32_store(CUtensorMap* tm, void* base, uint64_t inner, uint64_t rows) {
+// 2D fp16 tensor [rows, inner] for TMA stores of 64-column x 32-row boxes (128-byte rows, 128B swizzle).
+slp_status make_tmap_f16_store(CUtensorMap* tm, void* base, uint64_t inner, uint64_t rows) {
   EncodeTiledFn fn = get_encode_fn();
   if (!fn) return fail(SLP_ERR_CUDA, "cuTensorMapEncodeTiled not available from the driver");
   cuuint64_t dims[2] = {inner, rows};
-  cuuint64_t strides[1] = {inner * 4};
-  cuuint32_t box[2] = {32, 32};
+  cuuint64_t strides[1] = {inner * 2};
+  cuuint32_t box[2] = {64, 32};
   cuuint32_t estr[2] = {1, 1};
-  CUresult r = fn(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+  CUresult r = fn(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                   CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return fail(SLP_ERR_CUDA, "cuTensorMapEncodeTiled (Y store) failed with CUresult %d", static_cast<int>(r));
   return SLP_OK;
@@ -185,7 +185,9 @@ struct slp_moe_layer {
           *d_tile_expert = nullptr, *d_pos = nullptr, *d_row_token = nullptr, *d_pair_start = nullptr, *d_pair_expert = nullptr;
   int4* d_tile_info = nullptr;
   uint8_t *d_xq = nullptr, *d_hq = nullptr;
-  float* d_y = nullptr;
+  uint16_t* d_y = nullptr;  // [rows, H] fp16 per-row expert outputs, block-scaled by d_ys
+  float* d_ys = nullptr;    // [rows, ys_stride] power-of-two scale per row per 128 columns
+  int ys_stride = 0;
   int* d_err = nullptr;
   unsigned long long* d_clk = nullptr;
   int* d_sched = nullptr;
@@ -406,6 +408,8 @@ slp::GemmArgs gemm_args(L* h, int mode, int e_begin, int e_end, int T) {
   g.hs = h->d_hs;
   g.hs_stride = h->hs_stride;
   g.y = h->d_y;
+  g.ys = h->d_ys;
+  g.ys_stride = h->ys_stride;
   g.err = h->d_err;
   g.clk = h->d_clk;
   g.sched = h->d_sched;
@@ -639,7 +643,7 @@ slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t
   }
   CU_TRY(cudaEventRecord(h->ev_t[3], s));
   // ---- a9 combine ----
-  slp::combine_kernel<<<T, 256, 0, s>>>(h->d_y, h->d_pos, h->d_w, static_cast<__nv_bfloat16*>(out), T, H, k, shared ? 1 : 0);
+  slp::combine_kernel<<<T, 256, 0, s>>>(h->d_y, h->d_ys, h->d_pos, h->d_w, static_cast<__nv_bfloat16*>(out), T, H, k, shared ? 1 : 0, h->ys_stride);
   launched(1);
   CU_TRY(cudaGetLastError());
   CU_TRY(cudaMemcpyAsync(h->h_err, h->d_err, sizeof(int), cudaMemcpyDeviceToHost, s));
@@ -693,6 +697,7 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
   h->kbH = H / 128; h->kbI = I / 128;
   h->xs_stride = round_up(h->kbH, 4);
   h->hs_stride = round_up(h->kbI, 4);
+  h->ys_stride = round_up(h->kbH, 4);
   h->num_sms = prop.multiProcessorCount;
   h->slot_bytes = static_cast<size_t>(3) * I * H;
   const int Tpad = round_up(h->Tm, 128);
@@ -802,7 +807,8 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
   CU_OR_BAIL(cudaMalloc(&h->d_xs, rows * h->xs_stride * sizeof(float)));
   CU_OR_BAIL(cudaMalloc(&h->d_hq, rows * I));
   CU_OR_BAIL(cudaMalloc(&h->d_hs, rows * h->hs_stride * sizeof(float)));
-  CU_OR_BAIL(cudaMalloc(&h->d_y, rows * H * sizeof(float)));
+  CU_OR_BAIL(cudaMalloc(&h->d_y, rows * H * sizeof(uint16_t)));
+  CU_OR_BAIL(cudaMalloc(&h->d_ys, rows * h->ys_stride * sizeof(float)));
   CU_OR_BAIL(cudaMalloc(&h->d_clk, 4 * sizeof(unsigned long long)));
   CU_OR_BAIL(cudaMalloc(&h->d_sched, 2 * sizeof(int)));
   CU_OR_BAIL(cudaMalloc(&h->d_err, sizeof(int)));
@@ -819,7 +825,7 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
 
   TRY_OR_BAIL(make_tmap_u8(&h->tm_xq, h->d_xq, H, rows));
   TRY_OR_BAIL(make_tmap_u8(&h->tm_hq, h->d_hq, I, rows));
-  TRY_OR_BAIL(make_tmap_f32_store(&h->tm_y, h->d_y, H, rows));
+  TRY_OR_BAIL(make_tmap_f16_store(&h->tm_y, h->d_y, H, rows));
   TRY_OR_BAIL(alloc_pool(h, n_stage, epl));
 
   CU_OR_BAIL(cudaFuncSetAttribute(slp::tc::gemm_tc_kernel<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::tc::Cfg<0, true>::kSmemBytes));
@@ -855,7 +861,7 @@ slp_status slp_moe_query_plan(const slp_moe_cfg* cfg, slp_moe_plan* plan) {
   plan->pool_bytes_streamed = (1 + n_stage) * 3 * I * H;
   plan->pool_bytes_resident = (1 + E) * 3 * I * H;
   plan->scale_bytes = (E + 1) * (2 * (I / 128) * (H / 128) + (H / 128) * (I / 128)) * 4;
-  plan->workspace_bytes = rows * (H + xs_stride * 4 + I + hs_stride * 4 + H * 4 + 4) + Tm * (E * 4 + k * 12);
+  plan->workspace_bytes = rows * (H + xs_stride * 4 + I + hs_stride * 4 + H * 2 + xs_stride * 4 + 4) + Tm * (E * 4 + k * 12);
   plan->fp8_flops_per_token = 2 * 3 * I * H * (k + cfg->n_shared);
   plan->gemm_smem_bytes_gateup = slp::tc::Cfg<0, false>::kSmemBytes;
   plan->gemm_smem_bytes_down = slp::tc::Cfg<1, false>::kSmemBytes;
@@ -957,7 +963,7 @@ slp_status slp_moe_layer_destroy(slp_moe_layer* h) {
   free_pool(h);
   void* ptrs[] = {h->d_router_hl, h->d_router_w, h->d_bias, h->d_gate_s, h->d_up_s, h->d_down_s, h->d_logits, h->d_w, h->d_xs, h->d_hs, h->d_idx,
                   h->d_counts, h->d_chunk, h->d_row_start, h->d_tile_start, h->d_tile_expert, h->d_pair_start, h->d_pair_expert, h->d_tile_info, h->d_pos, h->d_row_token, h->d_xq,
-                  h->d_hq, h->d_y, h->d_err, h->d_clk, h->d_sched, h->d_e2e_in, h->d_e2e_out};
+                  h->d_hq, h->d_y, h->d_ys, h->d_err, h->d_clk, h->d_sched, h->d_e2e_in, h->d_e2e_out};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   if (h->h_counts) cudaFreeHost(h->h_counts);
@@ -1014,8 +1020,9 @@ slp_status locate_buffer(slp_moe_layer* h, int32_t which, const void** src, size
     case SLP_BUF_ROW_TOKEN: *src = h->d_row_token; *size = rows * sizeof(int32_t); break;
     case SLP_BUF_HQ: *src = h->d_hq; *size = rows * h->I; break;
     case SLP_BUF_HS: *src = h->d_hs; *size = rows * h->hs_stride * sizeof(float); break;
-    case SLP_BUF_Y: *src = h->d_y; *size = rows * h->H * sizeof(float); break;
+    case SLP_BUF_Y: *src = h->d_y; *size = rows * h->H * sizeof(uint16_t); break;
     case SLP_BUF_LOGITS: *src = h->d_logits; *size = T * h->E * sizeof(float); break;
+    case SLP_BUF_YS: *src = h->d_ys; *size = rows * h->ys_stride * sizeof(float); break;
     default: return fail(SLP_ERR_INVALID_ARG, "unknown buffer id %d", which);
   }
   return SLP_OK;

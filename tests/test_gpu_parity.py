@@ -14,6 +14,7 @@ import torch
 from oracle import moe_layer, permutation
 from oracle.acceptance import compare_routing, compare_output
 from paper_2606_10493_b200 import SlpMoeLayer, SlpError, inputs
+from gpu_util import read_y_rows, y_tolerance
 
 pytestmark = pytest.mark.gpu
 
@@ -173,7 +174,8 @@ def test_expert_intermediates_against_oracle(name, triage):
         hs_stride = (cfg.I // 128 + 3) // 4 * 4
         hq = layer.debug_buffer("hq", np.uint8).reshape(-1, cfg.I)
         hs = layer.debug_buffer("hs", np.float32).reshape(-1, hs_stride)[:, :cfg.I // 128]
-        y = layer.debug_buffer("y", np.float32).reshape(-1, cfg.H)
+        n_rows = hq.shape[0]
+        y = read_y_rows(layer, cfg, 0, n_rows)
     finally:
         layer.close()
     assert np.array_equal(xq, ref["xq"]) and np.array_equal(xs, ref["xs"])
@@ -203,7 +205,7 @@ def test_expert_intermediates_against_oracle(name, triage):
         # so a flipped code upstream does not blur the check: only fp32 accumulation noise is left
         y_own = dequantize_rows_1x128(g_hq, g_hs) @ dequantize_weight_128x128(ws[4], ws[5]).T
         rms = np.sqrt((y_own ** 2).mean())
-        assert np.abs(g_y - y_own).max() <= 2e-5 * rms + 1e-30, (e, np.abs(g_y - y_own).max() / rms)
+        assert (np.abs(g_y - y_own) <= y_tolerance(y_own, rms)).all(), (e, np.abs(g_y - y_own).max() / rms)
     print(name, triage, "codes", n_codes, "differ", n_flip)
     assert n_flip <= 1e-4 * n_codes   # observed: 4 of 718 848 (accumulation-order noise, SURVEY.md Q21 predicts ~2e-5)
 
