@@ -78,6 +78,11 @@ typedef struct {
                                  prefill).  0: paper-faithful fixed order, every expert copied. */
   int32_t require_pinned;     /* 1: create fails with SLP_ERR_NOT_PINNED if a weight buffer is
                                  pageable.  0: create pins it with cudaHostRegister. */
+  int32_t expert_begin;       /* Expert sharding (the paper's SmallEP): this handle owns the routed */
+  int32_t expert_end;         /* experts [expert_begin, expert_end).  0, 0 = all E.  A sharded handle still routes every
+                                 token over all E experts, but copies, stores and runs only its own experts; the host
+                                 pointers of the other experts may be NULL.  It is driven through
+                                 slp_moe_prefill_partial; staging_slots counts this handle's experts. */
 } slp_moe_cfg;
 
 /* Host weight pointers.  Borrowed for the lifetime of the handle; the host copy stays
@@ -192,6 +197,21 @@ slp_status slp_moe_set_residency(slp_moe_layer* h, slp_residency r);
  *  watchdog, this call returns SLP_ERR_KERNEL_TIMEOUT and enqueues nothing.
  *  With skip_empty_experts == 1 the call synchronises cuda_stream once internally. */
 slp_status slp_moe_prefill(slp_moe_layer* h, const void* hidden_bf16, int32_t T, void* out_bf16, void* cuda_stream);
+
+/* SmallEP step 2-4 on one rank ("every rank gates and sorts the full batch locally and keeps only
+ * tokens for its local experts ... executes its local experts and produces a partial weighted sum of shape [N, D]").
+ *  hidden_bf16: dev [T, H], the ALL-GATHERED hidden states of all ranks (same on every rank).
+ *  partial_f32: dev [T, H] fp32, fully overwritten with  sum over this handle's experts of w[t,j] * FFN(hidden[t])
+ *  for every token, plus FFN_shared(hidden[t]) for tokens t in [shared_token_begin, shared_token_end) only (the
+ *  shared expert is token-sharded; an empty range leaves it out).  No bf16 rounding: the ranks' partial sums are
+ *  added first (reduce-scatter) and rounded once by slp_moe_finalize_partial.  Works on an unsharded handle too
+ *  (then the partial sum is the whole layer in fp32).  Ordering, copy stream and error rules as slp_moe_prefill. */
+slp_status slp_moe_prefill_partial(slp_moe_layer* h, const void* hidden_bf16, int32_t T, float* partial_f32,
+                                   int32_t shared_token_begin, int32_t shared_token_end, void* cuda_stream);
+
+/* out_bf16[i] = bf16_rne(sum_f32[i]) for n_elems elements (multiple of 4) on `device`: the single output rounding
+ * of the SmallEP path, applied to the reduce-scattered sum.  Asynchronous on cuda_stream. */
+slp_status slp_moe_finalize_partial(int32_t device, const float* sum_f32, size_t n_elems, void* out_bf16, void* cuda_stream);
 
 /* End-to-end convenience: same as slp_moe_prefill but hidden/out are HOST buffers ([T,H] bf16,
  * pinned for full speed); copies in and out through an internal device buffer on the internal

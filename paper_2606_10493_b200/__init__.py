@@ -6,7 +6,7 @@ loudly if it has not been built (`python __graft_entry__.py` builds it); there i
 PyTorch fallback for any step of the path.
 """
 
-from . import inputs, sharding  # noqa: F401
+from . import inputs, sharding, smallep  # noqa: F401
 from .binding import (  # noqa: F401
-    SlpMoeLayer, SlpError, lib, library_path, measure_h2d_gbs, query_plan, EXPORTED_SYMBOLS,
+    SlpMoeLayer, SlpError, lib, library_path, measure_h2d_gbs, query_plan, finalize_partial, EXPORTED_SYMBOLS,
 )

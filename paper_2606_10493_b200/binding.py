@@ -16,6 +16,7 @@ EXPORTED_SYMBOLS = [
     "slp_moe_layer_destroy", "slp_last_error", "slp_moe_debug_routing",
     "slp_moe_debug_quant_hidden", "slp_moe_debug_buffer", "slp_moe_get_stats",
     "slp_measure_h2d", "slp_version", "slp_moe_query_plan", "slp_moe_debug_buffer_range",
+    "slp_moe_prefill_partial", "slp_moe_finalize_partial",
 ]
 
 SLP_STREAMED, SLP_RESIDENT = 0, 1
@@ -37,7 +38,7 @@ class _Cfg(C.Structure):
                 ("scoring", C.c_int32), ("norm_topk", C.c_int32), ("routed_scale", C.c_float),
                 ("max_tokens", C.c_int32), ("staging_slots", C.c_int32),
                 ("experts_per_launch", C.c_int32), ("skip_empty_experts", C.c_int32),
-                ("require_pinned", C.c_int32)]
+                ("require_pinned", C.c_int32), ("expert_begin", C.c_int32), ("expert_end", C.c_int32)]
 
 
 class _HostWeights(C.Structure):
@@ -82,6 +83,8 @@ def lib():
         L.slp_moe_layer_create.argtypes = [C.POINTER(_Cfg), C.POINTER(_HostWeights), C.POINTER(C.c_void_p)]
         L.slp_moe_set_residency.argtypes = [C.c_void_p, C.c_int]
         L.slp_moe_prefill.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
+        L.slp_moe_prefill_partial.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p]
+        L.slp_moe_finalize_partial.argtypes = [C.c_int32, C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p]
         L.slp_moe_prefill_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
         L.slp_moe_layer_destroy.argtypes = [C.c_void_p]
         L.slp_moe_debug_routing.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -108,12 +111,13 @@ def measure_h2d_gbs(device=0, chunk_bytes=44040192, total_bytes=1 << 30, repeats
     return out.value
 
 
-def _ptr_array(tensor):
-    """E pointers to the per-expert slices of a host tensor with leading expert axis."""
-    n = tensor.shape[0]
+def _ptr_array(tensor, n_experts=None, offset=0):
+    """E pointers to the per-expert slices of a host tensor with leading expert axis.  `offset`: the
+    tensor holds experts offset .. offset + len - 1 only (an expert shard); the other entries are NULL."""
+    n = max(tensor.shape[0] + offset, n_experts or 0, 1)
     arr = (C.c_void_p * n)()
-    for e in range(n):
-        arr[e] = tensor[e].data_ptr()
+    for e in range(tensor.shape[0]):
+        arr[offset + e] = tensor[e].data_ptr()
     return arr
 
 
@@ -130,14 +134,15 @@ class Plan(C.Structure):
 
 
 def _make_cfg(cfg, *, max_tokens=None, device=0, staging_slots=0, experts_per_launch=0, skip_empty_experts=False,
-              require_pinned=False):
+              require_pinned=False, expert_range=None):
     return _Cfg(struct_size=C.sizeof(_Cfg), device=device, hidden=cfg.H, n_experts=cfg.E,
                 top_k=cfg.k, n_group=cfg.G, topk_group=cfg.Gk, moe_intermediate=cfg.I,
                 n_shared=cfg.n_shared, shared_intermediate=cfg.I if cfg.n_shared else 0,
                 scoring=SCORING[cfg.scoring], norm_topk=int(cfg.norm_topk),
                 routed_scale=cfg.routed_scale, max_tokens=max_tokens or cfg.T,
                 staging_slots=staging_slots, experts_per_launch=experts_per_launch,
-                skip_empty_experts=int(skip_empty_experts), require_pinned=int(require_pinned))
+                skip_empty_experts=int(skip_empty_experts), require_pinned=int(require_pinned),
+                expert_begin=expert_range[0] if expert_range else 0, expert_end=expert_range[1] if expert_range else 0)
 
 
 def query_plan(cfg, **kw):
@@ -149,23 +154,39 @@ def query_plan(cfg, **kw):
     return plan.as_dict()
 
 
+def finalize_partial(sum_f32, out=None, stream=None):
+    """slp_moe_finalize_partial: bf16_rne of a reduced fp32 partial sum (CUDA tensors)."""
+    import torch
+    assert sum_f32.is_cuda and sum_f32.dtype == torch.float32 and sum_f32.is_contiguous()
+    if out is None:
+        out = torch.empty(sum_f32.shape, dtype=torch.bfloat16, device=sum_f32.device)
+    s = torch.cuda.current_stream(sum_f32.device) if stream is None else stream
+    _check(lib().slp_moe_finalize_partial(sum_f32.device.index, sum_f32.data_ptr(), sum_f32.numel(), out.data_ptr(), s.cuda_stream))
+    return out
+
+
 class SlpMoeLayer:
     """One MoE layer handle.  `weights` is the dict `inputs.make_weights` returns (host torch
     tensors, kept alive by this object because the library borrows the memory)."""
 
     def __init__(self, cfg, weights, *, max_tokens=None, device=0, staging_slots=0,
-                 experts_per_launch=0, skip_empty_experts=False, require_pinned=False, triage=None):
-        """`triage`: value for the library's SLP_TRIAGE environment switch during create (e.g.
-        "gemm=simt", "gemm=pair,router=fp32"); bring-up / bisection only, not part of the ABI."""
+                 experts_per_launch=0, skip_empty_experts=False, require_pinned=False, triage=None, expert_range=None):
+        """`expert_range` = (e0, e1): the handle owns routed experts [e0, e1) only (SmallEP); `weights` may then
+        hold just that shard (inputs.make_weights(..., shard=(e0, e1))).  `triage`: value for the library's
+        SLP_TRIAGE environment switch during create (e.g. "gemm=simt", "gemm=pair,router=fp32"); bring-up /
+        bisection only, not part of the ABI."""
         self._h = C.c_void_p()
         self.cfg = cfg
         self.weights = weights
         self.max_tokens = max_tokens or cfg.T
+        self.expert_range = tuple(expert_range) if expert_range else None
+        self.device = device
         c = _make_cfg(cfg, max_tokens=self.max_tokens, device=device, staging_slots=staging_slots,
                       experts_per_launch=experts_per_launch, skip_empty_experts=skip_empty_experts,
-                      require_pinned=require_pinned)
+                      require_pinned=require_pinned, expert_range=self.expert_range)
         w = weights
-        self._arrays = {k: _ptr_array(w[k]) for k in ("gate_q", "gate_s", "up_q", "up_s", "down_q", "down_s")}
+        off = w.get("expert_offset", 0)
+        self._arrays = {k: _ptr_array(w[k], cfg.E, off) for k in ("gate_q", "gate_s", "up_q", "up_s", "down_q", "down_s")}
 
         def p(t):
             return None if t is None else t.data_ptr()
@@ -202,6 +223,19 @@ class SlpMoeLayer:
         s = torch.cuda.current_stream(hidden.device) if stream is None else stream
         _check(lib().slp_moe_prefill(self._h, hidden.data_ptr(), hidden.shape[0], out.data_ptr(), s.cuda_stream))
         return out
+
+    def prefill_partial(self, hidden_all, partial=None, shared_tokens=(0, 0), stream=None):
+        """SmallEP: hidden_all = the all-gathered CUDA bf16 [T, H] hidden states; returns the fp32 [T, H] partial
+        weighted sum over this handle's experts (+ the shared expert for tokens in `shared_tokens`)."""
+        import torch
+        assert hidden_all.is_cuda and hidden_all.dtype == torch.bfloat16 and hidden_all.is_contiguous()
+        if partial is None:
+            partial = torch.empty(hidden_all.shape, dtype=torch.float32, device=hidden_all.device)
+        assert partial.dtype == torch.float32 and partial.is_contiguous() and partial.shape == hidden_all.shape
+        s = torch.cuda.current_stream(hidden_all.device) if stream is None else stream
+        _check(lib().slp_moe_prefill_partial(self._h, hidden_all.data_ptr(), hidden_all.shape[0], partial.data_ptr(),
+                                             int(shared_tokens[0]), int(shared_tokens[1]), s.cuda_stream))
+        return partial
 
     def prefill_host(self, hidden_host, out_host):
         """hidden_host/out_host: HOST bf16 [T, H] tensors (pinned for full speed).  Blocking."""

@@ -22,7 +22,9 @@ struct GemmArgs {
   const int32_t* pair_expert;  // [pairs] expert of each pair of 128-row tiles
   int e_begin, e_end;          // experts covered by this launch: [e_begin, e_end), E = shared
   int E, T;
-  int n_stage;                 // slot of routed expert e is 1 + e % n_stage; shared expert: slot 0
+  int e_own0;                  // first routed expert this handle owns (SmallEP expert sharding; 0 on one GPU)
+  int shared_rows;             // rows of the shared expert's token range (T on one GPU)
+  int n_stage;                 // slot of routed expert e is 1 + (e - e_own0) % n_stage; shared expert: slot 0
   int n_slots;                 // 1 + n_stage slots per weight kind: pool = [gate slots | up slots | down slots]
   // operands
   const uint8_t* a_q;          // [rows, K] e4m3
@@ -45,8 +47,8 @@ struct GemmArgs {
   unsigned long long* clk;     // [4] {SM cycles, ns} of CTA 0 summed over gate/up launches, then over down launches
 };
 
-__device__ __forceinline__ int slot_of(const GemmArgs& g, int e) { return e == g.E ? 0 : 1 + e % g.n_stage; }
-__device__ __forceinline__ int rows_of(const GemmArgs& g, int e) { return e == g.E ? g.T : g.counts[e]; }
+__device__ __forceinline__ int slot_of(const GemmArgs& g, int e) { return e == g.E ? 0 : 1 + (e - g.e_own0) % g.n_stage; }
+__device__ __forceinline__ int rows_of(const GemmArgs& g, int e) { return e == g.E ? g.shared_rows : g.counts[e]; }
 
 __device__ __forceinline__ float e4m3_to_float(uint8_t c) {
   __half_raw h = __nv_cvt_fp8_to_halfraw(c, __NV_E4M3);

@@ -347,11 +347,21 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
     Tile nx{0, 0, 0, 0};
     if (w_first < total) { nx = fetch(w_first); open_tile(nx); }
     int w = w_first < total ? w_first : -1;
+#ifdef SLP_PROF
+    long long pk = 0, pe = 0, pf = 0, pn = 0, pq = 0;
+#endif
     for (int i = 0; w >= 0; ++i, tile_parity ^= 1) {
+#ifdef SLP_PROF
+      const long long p0 = clock64();
+      long long p1 = p0;
+#endif
       const Tile cur = nx;
       w = next_item(w, i, true);
       const bool has_next = w >= 0;
       if (has_next) nx = fetch(w);  // record in flight during the K loop
+#ifdef SLP_PROF
+      const long long pa = clock64();
+#endif
       const int nt = cur.nt, row0 = cur.row0, nrows = cur.nrows;
       const size_t row = static_cast<size_t>(row0 + r_in_tile);
       const bool row_ok_cur = row_ok;
@@ -390,12 +400,17 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
           const uint32_t buf = it & 1;
           ptx::mbar_wait_a(bar_a + kOffTmemFull + 8 * buf, (it >> 1) & 1, dead, g.err, 4);
           ptx::tc_fence_after();
+#ifdef SLP_PROF
+          if (kb == 0) p1 = clock64();
+#endif
           const uint32_t tb = tm_lane + buf * BN;
-          if constexpr (kPair) {
+          {
             // 8 chunks of 16 columns through four register sets: chunks 0-3 are loaded up front, chunk
             // c + 4 is requested as soon as the FMAs of chunk c have consumed its set, so every
             // tcgen05.ld of the K block has landed after half of the FMAs and the TMEM buffer goes back
-            // to the MMA issuer there (the hand-off round trip, not throughput, bounds the kernel).
+            // to the MMA issuer there.  The K loop is bound by the hand-off round trip, not by throughput:
+            // time per K block = (MMA 512 + ~500 cycles of commit / wake-up / issue latency + drain) / 2
+            // with two TMEM buffers, drain = buffer published -> buffer released.
             uint32_t v[4][16];
   #pragma unroll
             for (int c = 0; c < 4; ++c) ptx::tmem_ld16(tb + c * 16, v[c]);
@@ -423,41 +438,13 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
   #pragma unroll
               for (int i = 0; i < 16; i += 2) ptx::fma2(acc2[(c + 4) * 8 + i / 2], v[c][i], v[c][i + 1], s2);
             }
-          } else {
-            // 8 chunks of 16 columns, two register sets in flight; one FFMA2 per column pair
-            uint32_t v0[16], v1[16];
-            ptx::tmem_ld16(tb, v0);
-  #pragma unroll
-            for (int c = 0; c < 8; c += 2) {
-              ptx::tmem_ld_wait();
-              ptx::tmem_ld16(tb + (c + 1) * 16, v1);
-              {
-                const uint64_t s2 = (c < 4) ? s20 : s21;
-  #pragma unroll
-                for (int i = 0; i < 16; i += 2) ptx::fma2(acc2[c * 8 + i / 2], v0[i], v0[i + 1], s2);
-              }
-              ptx::tmem_ld_wait();
-              if (c + 2 < 8) {
-                ptx::tmem_ld16(tb + (c + 2) * 16, v0);
-              } else {
-                // the whole partial is in registers: hand the TMEM buffer back before the last FMAs
-                ptx::tc_fence_before();
-                __syncwarp();
-                if (lane == 0) {
-                  if (kPair && rank != 0) ptx::mbar_arrive_cluster(te_a + 8 * buf);  // remote: the leader's barrier
-                  else ptx::mbar_arrive_a(bar_a + kOffTmemEmpty + 8 * buf);
-                }
-              }
-              {
-                const uint64_t s2 = (c + 1 < 4) ? s20 : s21;
-  #pragma unroll
-                for (int i = 0; i < 16; i += 2) ptx::fma2(acc2[(c + 1) * 8 + i / 2], v1[i], v1[i + 1], s2);
-              }
-            }
           }
           ++it;
         }
       }
+#ifdef SLP_PROF
+      const long long p2 = clock64();
+#endif
       if (has_next) open_tile(nx);  // first scale loads of the next tile fly during this tile's epilogue
       float acc[128];
 #pragma unroll
@@ -508,9 +495,13 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
         // the workspace; whole 32-row groups past it are skipped.
         const int c0 = nt * BN + half * HN;
         if (c0 < g.H && q * 32 < nrows) {
-          float amax = 0.f;
+          float am[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};  // eight independent chains instead of one of 128
 #pragma unroll
-          for (int i = 0; i < 128; ++i) amax = fmaxf(amax, fabsf(acc[i]));
+          for (int i = 0; i < 128; i += 16) {
+#pragma unroll
+            for (int u = 0; u < 8; ++u) am[u] = fmaxf(am[u], fmaxf(fabsf(acc[i + 2 * u]), fabsf(acc[i + 2 * u + 1])));
+          }
+          const float amax = fmaxf(fmaxf(fmaxf(am[0], am[1]), fmaxf(am[2], am[3])), fmaxf(fmaxf(am[4], am[5]), fmaxf(am[6], am[7])));
           const uint32_t eb = max(__float_as_uint(amax) >> 23, 14u);          // biased exponent of amax (>= 0)
           const float mult = __uint_as_float((268u - eb) << 23);                // 2^(14 - floor(log2 amax))
           g.ys[row * g.ys_stride + (c0 >> 7)] = __uint_as_float((eb - 14u) << 23);  // 2^(floor(log2 amax) - 14)
@@ -538,7 +529,19 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
           }
         }
       }
+#ifdef SLP_PROF
+      { const long long p3 = clock64(); pf += p1 - pa; pq += pa - p0; pk += p2 - p1; pe += p3 - p2; pn += 1; }
+#endif
     }
+#ifdef SLP_PROF
+    if (warp == 0 && lane == 0) {
+      atomicAdd(&g.clk[4 + 4 * kMode], static_cast<unsigned long long>(pf));
+      atomicAdd(&g.clk[5 + 4 * kMode], static_cast<unsigned long long>(pk));
+      atomicAdd(&g.clk[6 + 4 * kMode], static_cast<unsigned long long>(pe));
+      atomicAdd(&g.clk[7 + 4 * kMode], static_cast<unsigned long long>(pn));
+      atomicAdd(&g.clk[12 + kMode], static_cast<unsigned long long>(pq));
+    }
+#endif
     if (kMode == 1 && lane == 0) ptx::bulk_wait_group_read<0>();  // staging memory must outlive the last stores
   }
 

@@ -354,12 +354,16 @@ __global__ void __launch_bounds__(128) permute_hist_kernel(const int32_t* __rest
     for (int e = lane; e < E; e += 32) chunk_counts[static_cast<size_t>(chunk) * E + e] = h[e];
 }
 
+// Expert sharding (the paper's SmallEP: every rank gates and sorts the full batch and keeps only
+// the tokens of its own experts): experts outside [e_own0, e_own1) keep their true count in counts[] but get no
+// rows and no tiles.  The shared expert covers the token range [sh_t0, sh_t1) (all tokens on one GPU, this
+// rank's token shard under SmallEP, empty = no shared expert).
 __global__ void __launch_bounds__(512) permute_scan_kernel(int32_t* __restrict__ chunk_counts, int32_t* __restrict__ counts,
                                                            int32_t* __restrict__ row_start, int32_t* __restrict__ tile_start,
                                                            int32_t* __restrict__ tile_expert, int32_t* __restrict__ pair_start,
                                                            int32_t* __restrict__ pair_expert, int4* __restrict__ tile_info,
-                                                           int n_chunks, int T, int E, int has_shared) {
-  __shared__ int32_t s_cnt[kMaxExperts + 1];
+                                                           int n_chunks, int T, int E, int e_own0, int e_own1, int sh_t0, int sh_t1) {
+  __shared__ int32_t s_cnt[kMaxExperts + 1];   // rows that get workspace rows (0 for experts of other ranks)
   __shared__ int32_t s_tile[kMaxExperts + 2];
   __shared__ int32_t s_row[kMaxExperts + 2];
   __shared__ int32_t s_pair[kMaxExperts + 2];  // prefix of ceil(m tiles / 2): work items of the CTA-pair GEMM
@@ -376,7 +380,7 @@ __global__ void __launch_bounds__(512) permute_scan_kernel(int32_t* __restrict__
         run += v[u];
       }
     }
-    s_cnt[e] = run;
+    s_cnt[e] = (e >= e_own0 && e < e_own1) ? run : 0;
     counts[e] = run;
   }
   __syncthreads();
@@ -393,13 +397,14 @@ __global__ void __launch_bounds__(512) permute_scan_kernel(int32_t* __restrict__
       tile += mt;
       pair += (mt + 1) / 2;
     }
-    row_start[E] = 0;  // shared expert: the un-permuted rows
-    s_row[E] = 0;
-    s_cnt[E] = T;
+    const int sh_rows = max(0, sh_t1 - sh_t0), sh_tiles = (sh_rows + 127) / 128;
+    row_start[E] = sh_t0;  // shared expert: the un-permuted rows of its token range
+    s_row[E] = sh_t0;
+    s_cnt[E] = sh_rows;
     s_tile[E] = tile;
     s_pair[E] = pair;
-    tile += has_shared ? Tpad / 128 : 0;
-    pair += has_shared ? (Tpad / 128 + 1) / 2 : 0;
+    tile += sh_tiles;
+    pair += (sh_tiles + 1) / 2;
     s_tile[E + 1] = tile;
     s_pair[E + 1] = pair;
     row_start[E + 1] = row;  // total rows in use
@@ -418,7 +423,7 @@ __global__ void __launch_bounds__(512) permute_scan_kernel(int32_t* __restrict__
 
 __global__ void __launch_bounds__(128) permute_place_kernel(const int32_t* __restrict__ idx, const int32_t* __restrict__ chunk_off,
                                                             const int32_t* __restrict__ row_start, int32_t* __restrict__ pos,
-                                                            int32_t* __restrict__ row_token, int T, int k, int E) {
+                                                            int32_t* __restrict__ row_token, int T, int k, int E, int e_own0, int e_own1) {
   extern __shared__ int32_t sm_run[];  // [warps][E] next free row of each expert for this chunk
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int chunk = blockIdx.x * (blockDim.x >> 5) + warp;
@@ -435,15 +440,16 @@ __global__ void __launch_bounds__(128) permute_place_kernel(const int32_t* __res
     const int e = valid ? src[i] : -1 - lane;  // entries are token-major: ascending lane = ascending token
     const uint32_t peers = __match_any_sync(0xFFFFFFFFu, e);
     const int rank = __popc(peers & ((1u << lane) - 1));
-    int dst = 0;
-    if (valid) dst = run[e] + rank;
+    const bool own = valid && e >= e_own0 && e < e_own1;  // experts of other ranks get no row: pos = -1
+    int dst = -1;
+    if (own) dst = run[e] + rank;
     __syncwarp();
-    if (valid && rank == 0) run[e] += __popc(peers);
+    if (own && rank == 0) run[e] += __popc(peers);
     __syncwarp();
     if (valid) {
       const int t = t0 + i / k;
       pos[static_cast<size_t>(t0) * k + i] = dst;
-      row_token[dst] = t;
+      if (own) row_token[dst] = t;
     }
   }
   for (int i = lane; i < min(kChunkTokens, T - t0); i += 32) row_token[t0 + i] = t0 + i;  // shared rows
@@ -494,6 +500,7 @@ __global__ void __launch_bounds__(256) quant_scatter_kernel(const uint16_t* __re
     const uint2 q = make_uint2(quant4_e4m3(v[0], v[1], v[2], v[3], s), quant4_e4m3(v[4], v[5], v[6], v[7], s));
     if (on) {
       for (int j = 0; j <= k; ++j) {
+        if (dst[j] < 0) continue;  // expert owned by another rank (SmallEP): no row here
         const size_t row = dst[j];
         *reinterpret_cast<uint2*>(xq + row * H + kb * kBlock + l16 * 8) = q;
         if (l16 == 0) xs[row * xs_stride + kb] = s;
@@ -518,9 +525,14 @@ __device__ __forceinline__ void fma_f16x8(float (&acc)[8], float s, const uint4&
   }
 }
 
+// kPartial (SmallEP): slots whose expert lives on another rank have pos < 0 and are skipped, the shared
+// expert is added only for tokens in [sh_t0, sh_t1), and the fp32 sum is written unrounded: the ranks'
+// partial sums are reduced first ("partial weighted sum ... exchange and local reduction")
+// and rounded to bf16 once, by partial_to_bf16_kernel.
+template <bool kPartial>
 __global__ void __launch_bounds__(256) combine_kernel(const uint16_t* __restrict__ y, const float* __restrict__ ys, const int32_t* __restrict__ pos,
-                                                      const float* __restrict__ w, __nv_bfloat16* __restrict__ out, int T, int H,
-                                                      int k, int has_shared, int ys_stride) {
+                                                      const float* __restrict__ w, void* __restrict__ out, int T, int H,
+                                                      int k, int sh_t0, int sh_t1, int ys_stride) {
   const int t = blockIdx.x;
   __shared__ int32_t s_row[32];
   __shared__ float s_w[32];
@@ -529,9 +541,11 @@ __global__ void __launch_bounds__(256) combine_kernel(const uint16_t* __restrict
     s_w[threadIdx.x] = w[static_cast<size_t>(t) * k + threadIdx.x];
   }
   __syncthreads();
+  const bool has_shared = t >= sh_t0 && t < sh_t1;
   for (int c = threadIdx.x * 8; c < H; c += blockDim.x * 8) {  // 8 channels = one 16-byte load per row
     float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
     for (int j = 0; j < k; ++j) {
+      if (kPartial && s_row[j] < 0) continue;
       const size_t row = s_row[j];
       const uint4 v = *reinterpret_cast<const uint4*>(y + row * H + c);
       fma_f16x8(acc, s_w[j] * ys[row * ys_stride + (c >> 7)], v);  // power-of-two block scale: the product is exact
@@ -540,12 +554,27 @@ __global__ void __launch_bounds__(256) combine_kernel(const uint16_t* __restrict
       const uint4 v = *reinterpret_cast<const uint4*>(y + static_cast<size_t>(t) * H + c);
       fma_f16x8(acc, ys[static_cast<size_t>(t) * ys_stride + (c >> 7)], v);
     }
-    uint4 o;
-    __nv_bfloat162 p0 = __floats2bfloat162_rn(acc[0], acc[1]), p1 = __floats2bfloat162_rn(acc[2], acc[3]);
-    __nv_bfloat162 p2 = __floats2bfloat162_rn(acc[4], acc[5]), p3 = __floats2bfloat162_rn(acc[6], acc[7]);
-    o.x = *reinterpret_cast<uint32_t*>(&p0); o.y = *reinterpret_cast<uint32_t*>(&p1);
-    o.z = *reinterpret_cast<uint32_t*>(&p2); o.w = *reinterpret_cast<uint32_t*>(&p3);
-    *reinterpret_cast<uint4*>(out + static_cast<size_t>(t) * H + c) = o;
+    if (kPartial) {
+      float4* dst = reinterpret_cast<float4*>(static_cast<float*>(out) + static_cast<size_t>(t) * H + c);
+      dst[0] = make_float4(acc[0], acc[1], acc[2], acc[3]);
+      dst[1] = make_float4(acc[4], acc[5], acc[6], acc[7]);
+    } else {
+      uint4 o;
+      __nv_bfloat162 p0 = __floats2bfloat162_rn(acc[0], acc[1]), p1 = __floats2bfloat162_rn(acc[2], acc[3]);
+      __nv_bfloat162 p2 = __floats2bfloat162_rn(acc[4], acc[5]), p3 = __floats2bfloat162_rn(acc[6], acc[7]);
+      o.x = *reinterpret_cast<uint32_t*>(&p0); o.y = *reinterpret_cast<uint32_t*>(&p1);
+      o.z = *reinterpret_cast<uint32_t*>(&p2); o.w = *reinterpret_cast<uint32_t*>(&p3);
+      *reinterpret_cast<uint4*>(static_cast<__nv_bfloat16*>(out) + static_cast<size_t>(t) * H + c) = o;
+    }
+  }
+}
+
+// The one bf16 rounding of the SmallEP path: reduced fp32 partial sums -> bf16 (n a multiple of 4).
+__global__ void __launch_bounds__(256) partial_to_bf16_kernel(const float* __restrict__ sum, __nv_bfloat16* __restrict__ out, size_t n4) {
+  for (size_t i = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x; i < n4; i += static_cast<size_t>(gridDim.x) * blockDim.x) {
+    const float4 v = reinterpret_cast<const float4*>(sum)[i];
+    __nv_bfloat162 lo = __floats2bfloat162_rn(v.x, v.y), hi = __floats2bfloat162_rn(v.z, v.w);
+    reinterpret_cast<uint2*>(out)[i] = make_uint2(*reinterpret_cast<uint32_t*>(&lo), *reinterpret_cast<uint32_t*>(&hi));
   }
 }
 

@@ -144,12 +144,16 @@ slp_status validate_cfg(const slp_moe_cfg* cfg, int* n_stage_out, int* epl_out) 
     return fail(SLP_ERR_UNSUPPORTED_SHAPE, "n_shared must be 0 or 1 with shared_intermediate == moe_intermediate");
   if (cfg->scoring != SLP_SCORE_SIGMOID_BIAS && cfg->scoring != SLP_SCORE_SOFTMAX) return fail(SLP_ERR_INVALID_ARG, "unknown scoring %d", cfg->scoring);
   if (cfg->max_tokens <= 0) return fail(SLP_ERR_INVALID_ARG, "max_tokens must be positive");
-  int n_stage = cfg->staging_slots == 0 ? E : cfg->staging_slots;
-  if (n_stage < 2 && E >= 2) return fail(SLP_ERR_INVALID_ARG, "staging_slots must be 0 or 2..n_experts");
-  n_stage = std::min(n_stage, E);
+  if (cfg->expert_begin < 0 || cfg->expert_end < 0 || cfg->expert_end > E || (cfg->expert_end != 0 && cfg->expert_begin >= cfg->expert_end) ||
+      (cfg->expert_end == 0 && cfg->expert_begin != 0))
+    return fail(SLP_ERR_INVALID_ARG, "expert range [%d, %d) invalid for %d experts (0, 0 = all)", cfg->expert_begin, cfg->expert_end, E);
+  const int En = cfg->expert_end == 0 ? E : cfg->expert_end - cfg->expert_begin;  // experts this handle owns
+  int n_stage = cfg->staging_slots == 0 ? En : cfg->staging_slots;
+  if (n_stage < 2 && En >= 2) return fail(SLP_ERR_INVALID_ARG, "staging_slots must be 0 or 2..(owned experts)");
+  n_stage = std::min(n_stage, En);
   int epl = cfg->experts_per_launch;
-  if (epl == 0) epl = auto_epl(n_stage, E);
-  if (epl < 1 || epl > n_stage || (n_stage != E && (epl > n_stage / 2 || n_stage % epl)))
+  if (epl == 0) epl = auto_epl(n_stage, En);
+  if (epl < 1 || epl > n_stage || (n_stage != En && (epl > n_stage / 2 || n_stage % epl)))
     return fail(SLP_ERR_INVALID_ARG, "experts_per_launch %d invalid for %d staging slots (must divide it, <= half)", epl, n_stage);
   *n_stage_out = n_stage;
   *epl_out = epl;
@@ -165,6 +169,7 @@ struct slp_moe_layer {
   std::vector<const uint8_t*> gate_q, up_q, down_q;
   std::vector<void*> registered;  // host ranges pinned by create
   int H = 0, E = 0, k = 0, I = 0, Tm = 0;
+  int e0 = 0, e1 = 0;  // owned routed experts [e0, e1) (SmallEP); the whole layer on one GPU
   int kbH = 0, kbI = 0, xs_stride = 0, hs_stride = 0;
   int rows_max = 0, tiles_max = 0, n_chunks_max = 0;
   int num_sms = 0;
@@ -201,6 +206,7 @@ struct slp_moe_layer {
   std::vector<cudaEvent_t> ev_ready, ev_free;
   std::vector<char> free_recorded;
   cudaEvent_t ev_done = nullptr, ev_t[6] = {}, ev_copy0 = nullptr, ev_copy1 = nullptr;
+  int sh_rows = 0;  // rows of the shared expert's token range in the call being enqueued
   bool in_flight = false;
   bool dead = false;               // the expert pool could not be restored after a failed residency switch
   bool pool_needs_upload = false;  // resident pool was rebuilt after a failed switch: experts must be re-uploaded
@@ -393,6 +399,8 @@ slp::GemmArgs gemm_args(L* h, int mode, int e_begin, int e_end, int T) {
   g.e_end = e_end;
   g.E = h->E;
   g.T = T;
+  g.e_own0 = h->e0;
+  g.shared_rows = h->sh_rows;
   g.n_stage = h->n_stage;
   g.n_slots = 1 + h->n_stage;
   g.a_q = mode == 0 ? h->d_xq : h->d_hq;
@@ -489,9 +497,9 @@ slp_status copy_experts(L* h, int e0, int e1, const int32_t* counts /* NULL = al
       if (!wanted(e)) { ++e; continue; }
       int n = 1;  // experts e .. e + n - 1 in one copy
       while (e + n < e1 && wanted(e + n) && p[e + n] == p[e] + static_cast<size_t>(n) * IH &&
-             (e + n) % h->n_stage == e % h->n_stage + n)
+             (e + n - h->e0) % h->n_stage == (e - h->e0) % h->n_stage + n)
         ++n;
-      CU_TRY(cudaMemcpyAsync(region + static_cast<size_t>(1 + e % h->n_stage) * IH, p[e], static_cast<size_t>(n) * IH,
+      CU_TRY(cudaMemcpyAsync(region + static_cast<size_t>(1 + (e - h->e0) % h->n_stage) * IH, p[e], static_cast<size_t>(n) * IH,
                              cudaMemcpyHostToDevice, h->copy_stream));
       h->stats.h2d_copies += 1;
       e += n;
@@ -505,9 +513,15 @@ slp_status copy_experts(L* h, int e0, int e1, const int32_t* counts /* NULL = al
   return SLP_OK;
 }
 
-slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t s) {
+// `partial`: out is fp32 [T, H], the unrounded weighted sum over the owned experts (+ the shared expert for tokens
+// in [sh_t0, sh_t1)); otherwise out is bf16 [T, H] and the shared expert covers every token.
+slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t s, bool partial = false, int sh_t0 = 0, int sh_t1 = -1) {
   const int E = h->E, k = h->k, H = h->H;
-  const bool shared = h->cfg.n_shared != 0;
+  if (sh_t1 < 0) sh_t1 = T;
+  if (h->cfg.n_shared == 0) sh_t0 = sh_t1 = 0;
+  const bool shared = sh_t1 > sh_t0;
+  h->sh_rows = sh_t1 - sh_t0;
+  const int e_own0 = h->e0, e_own1 = h->e1;
   h->stats = slp_moe_stats{};
   h->stats.struct_size = sizeof(slp_moe_stats);
   h->stats.tokens = T;
@@ -516,7 +530,7 @@ slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t
   h->ev_k_used = 0;
   auto launched = [&](int n) { h->stats.kernel_launches += n; };
 
-  CU_TRY(cudaMemsetAsync(h->d_clk, 0, 4 * sizeof(unsigned long long), s));
+  CU_TRY(cudaMemsetAsync(h->d_clk, 0, 16 * sizeof(unsigned long long), s));
   CU_TRY(cudaEventRecord(h->ev_t[0], s));
   // ---- a1 router ----
   {
@@ -571,8 +585,8 @@ slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t
     CU_TRY(cudaMemsetAsync(h->d_row_token, 0xFF, static_cast<size_t>(h->rows_max) * sizeof(int32_t), s));
     slp::permute_hist_kernel<<<blocks, wpb * 32, sm, s>>>(h->d_idx, h->d_chunk, T, k, E);
     slp::permute_scan_kernel<<<1, 512, 0, s>>>(h->d_chunk, h->d_counts, h->d_row_start, h->d_tile_start, h->d_tile_expert, h->d_pair_start, h->d_pair_expert, h->d_tile_info, n_chunks, T,
-                                               E, shared ? 1 : 0);
-    slp::permute_place_kernel<<<blocks, wpb * 32, sm, s>>>(h->d_idx, h->d_chunk, h->d_row_start, h->d_pos, h->d_row_token, T, k, E);
+                                               E, e_own0, e_own1, sh_t0, sh_t1);
+    slp::permute_place_kernel<<<blocks, wpb * 32, sm, s>>>(h->d_idx, h->d_chunk, h->d_row_start, h->d_pos, h->d_row_token, T, k, E, e_own0, e_own1);
     launched(3);
   }
   // ---- a3 hidden quantisation + scatter into expert order ----
@@ -581,8 +595,8 @@ slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t
   CU_TRY(cudaGetLastError());
   CU_TRY(cudaEventRecord(h->ev_t[1], s));
 
-  const int Tpad_tiles = (T + 127) / 128;
-  const int routed_tiles_bound = (T * k) / 128 + E;
+  const int Tpad_tiles = (h->sh_rows + 127) / 128;
+  const int routed_tiles_bound = (T * k) / 128 + (e_own1 - e_own0);
   h->stats.m_tiles = 0;
 
   bool skip = h->cfg.skip_empty_experts != 0;
@@ -593,8 +607,16 @@ slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t
 
   CU_TRY(cudaEventRecord(h->ev_t[2], s));
   if (h->residency == SLP_RESIDENT) {
-    slp_status st = launch_experts(h, s, 0, shared ? E + 1 : E, T, routed_tiles_bound + (shared ? Tpad_tiles : 0));
-    if (st != SLP_OK) return st;
+    // one launch pair covers the owned routed experts and, when it is adjacent (e_own1 == E), the shared expert
+    if (e_own1 == E || !shared) {
+      slp_status st = launch_experts(h, s, e_own0, shared ? E + 1 : e_own1, T, routed_tiles_bound + (shared ? Tpad_tiles : 0));
+      if (st != SLP_OK) return st;
+    } else {
+      slp_status st = launch_experts(h, s, e_own0, e_own1, T, routed_tiles_bound);
+      if (st != SLP_OK) return st;
+      st = launch_experts(h, s, E, E + 1, T, Tpad_tiles);
+      if (st != SLP_OK) return st;
+    }
   } else {
     // ---- a4 streaming engine ----
     if (shared) {  // resident weights: runs while the first expert copies are in flight
@@ -604,8 +626,8 @@ slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t
     const int epl = h->epl;
     const int n_ring = static_cast<int>(h->ev_ready.size());
     bool first_copy = true;
-    for (int e0 = 0, grp = 0; e0 < E; e0 += epl, ++grp) {
-      const int e1 = std::min(E, e0 + epl);
+    for (int e0 = e_own0, grp = 0; e0 < e_own1; e0 += epl, ++grp) {
+      const int e1 = std::min(e_own1, e0 + epl);
       const int r = grp % n_ring;
       int need = 0, rows_bound = 0;
       for (int e = e0; e < e1; ++e) {
@@ -643,7 +665,8 @@ slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t
   }
   CU_TRY(cudaEventRecord(h->ev_t[3], s));
   // ---- a9 combine ----
-  slp::combine_kernel<<<T, 256, 0, s>>>(h->d_y, h->d_ys, h->d_pos, h->d_w, static_cast<__nv_bfloat16*>(out), T, H, k, shared ? 1 : 0, h->ys_stride);
+  if (partial) slp::combine_kernel<true><<<T, 256, 0, s>>>(h->d_y, h->d_ys, h->d_pos, h->d_w, out, T, H, k, sh_t0, sh_t1, h->ys_stride);
+  else slp::combine_kernel<false><<<T, 256, 0, s>>>(h->d_y, h->d_ys, h->d_pos, h->d_w, out, T, H, k, sh_t0, sh_t1, h->ys_stride);
   launched(1);
   CU_TRY(cudaGetLastError());
   CU_TRY(cudaMemcpyAsync(h->h_err, h->d_err, sizeof(int), cudaMemcpyDeviceToHost, s));
@@ -694,6 +717,8 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
   h->triage = read_triage();
   h->hw = *w;
   h->H = H; h->E = E; h->k = k; h->I = I; h->Tm = cfg->max_tokens;
+  h->e0 = cfg->expert_end == 0 ? 0 : cfg->expert_begin;
+  h->e1 = cfg->expert_end == 0 ? E : cfg->expert_end;
   h->kbH = H / 128; h->kbI = I / 128;
   h->xs_stride = round_up(h->kbH, 4);
   h->hs_stride = round_up(h->kbI, 4);
@@ -729,7 +754,7 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
 
   // pin (or check) the streamed weights
   const size_t IH = static_cast<size_t>(I) * H;
-  for (int e = 0; e < E; ++e)
+  for (int e = h->e0; e < h->e1; ++e)
     if (!h->gate_q[e] || !h->up_q[e] || !h->down_q[e] || !w->gate_s[e] || !w->up_s[e] || !w->down_s[e])
       return bail(fail(SLP_ERR_INVALID_ARG, "NULL weight pointer for expert %d", e));
   {
@@ -739,9 +764,9 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
     const char* names[3] = {"gate_q", "up_q", "down_q"};
     for (int kind = 0; kind < 3; ++kind) {
       const std::vector<const uint8_t*>& p = *kinds[kind];
-      for (int e = 0; e < E;) {
+      for (int e = h->e0; e < h->e1;) {
         int n = 1;
-        while (e + n < E && p[e + n] == p[e] + static_cast<size_t>(n) * IH) ++n;
+        while (e + n < h->e1 && p[e + n] == p[e] + static_cast<size_t>(n) * IH) ++n;
         TRY_OR_BAIL(pin_range(h, p[e], static_cast<size_t>(n) * IH, names[kind]));
         e += n;
       }
@@ -777,7 +802,7 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
   CU_OR_BAIL(cudaMalloc(&h->d_gate_s, (E + 1) * sc_gu * sizeof(float)));
   CU_OR_BAIL(cudaMalloc(&h->d_up_s, (E + 1) * sc_gu * sizeof(float)));
   CU_OR_BAIL(cudaMalloc(&h->d_down_s, (E + 1) * sc_d * sizeof(float)));
-  for (int e = 0; e < E; ++e) {
+  for (int e = h->e0; e < h->e1; ++e) {
     CU_OR_BAIL(cudaMemcpy(h->d_gate_s + e * sc_gu, w->gate_s[e], sc_gu * sizeof(float), cudaMemcpyHostToDevice));
     CU_OR_BAIL(cudaMemcpy(h->d_up_s + e * sc_gu, w->up_s[e], sc_gu * sizeof(float), cudaMemcpyHostToDevice));
     CU_OR_BAIL(cudaMemcpy(h->d_down_s + e * sc_d, w->down_s[e], sc_d * sizeof(float), cudaMemcpyHostToDevice));
@@ -809,7 +834,7 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
   CU_OR_BAIL(cudaMalloc(&h->d_hs, rows * h->hs_stride * sizeof(float)));
   CU_OR_BAIL(cudaMalloc(&h->d_y, rows * H * sizeof(uint16_t)));
   CU_OR_BAIL(cudaMalloc(&h->d_ys, rows * h->ys_stride * sizeof(float)));
-  CU_OR_BAIL(cudaMalloc(&h->d_clk, 4 * sizeof(unsigned long long)));
+  CU_OR_BAIL(cudaMalloc(&h->d_clk, 16 * sizeof(unsigned long long)));
   CU_OR_BAIL(cudaMalloc(&h->d_sched, 2 * sizeof(int)));
   CU_OR_BAIL(cudaMalloc(&h->d_err, sizeof(int)));
   CU_OR_BAIL(cudaMemset(h->d_err, 0, sizeof(int)));
@@ -854,12 +879,13 @@ slp_status slp_moe_query_plan(const slp_moe_cfg* cfg, slp_moe_plan* plan) {
   const int64_t xs_stride = (H / 128 + 3) / 4 * 4, hs_stride = (I / 128 + 3) / 4 * 4;
   plan->staging_slots = n_stage;
   plan->experts_per_launch = epl;
-  plan->launch_pairs_streamed = static_cast<int32_t>((E + epl - 1) / epl + (cfg->n_shared ? 1 : 0));
+  const int64_t En = cfg->expert_end == 0 ? E : cfg->expert_end - cfg->expert_begin;
+  plan->launch_pairs_streamed = static_cast<int32_t>((En + epl - 1) / epl + (cfg->n_shared ? 1 : 0));
   plan->workspace_rows = rows;
   plan->expert_slot_bytes = 3 * I * H;
-  plan->routed_bytes_per_pass = E * 3 * I * H;
+  plan->routed_bytes_per_pass = En * 3 * I * H;
   plan->pool_bytes_streamed = (1 + n_stage) * 3 * I * H;
-  plan->pool_bytes_resident = (1 + E) * 3 * I * H;
+  plan->pool_bytes_resident = (1 + En) * 3 * I * H;
   plan->scale_bytes = (E + 1) * (2 * (I / 128) * (H / 128) + (H / 128) * (I / 128)) * 4;
   plan->workspace_bytes = rows * (H + xs_stride * 4 + I + hs_stride * 4 + H * 2 + xs_stride * 4 + 4) + Tm * (E * 4 + k * 12);
   plan->fp8_flops_per_token = 2 * 3 * I * H * (k + cfg->n_shared);
@@ -878,7 +904,7 @@ slp_status slp_moe_set_residency(slp_moe_layer* h, slp_residency r) {
   if (h->dead) return fail(SLP_ERR_OOM, "handle lost its expert pool in an earlier failed residency switch; destroy it");
   auto upload_all = [&]() -> slp_status {
     h->stats = slp_moe_stats{};
-    slp_status u = copy_experts(h, 0, h->E, nullptr);
+    slp_status u = copy_experts(h, h->e0, h->e1, nullptr);
     if (u != SLP_OK) return u;
     CU_TRY(cudaStreamSynchronize(h->copy_stream));
     h->pool_needs_upload = false;
@@ -889,14 +915,15 @@ slp_status slp_moe_set_residency(slp_moe_layer* h, slp_residency r) {
     return SLP_OK;
   }
   if (r == SLP_RESIDENT) {
-    st = alloc_pool(h, h->E, h->E);
+    st = alloc_pool(h, h->e1 - h->e0, h->e1 - h->e0);
     if (st != SLP_OK) return st;   // the handle is unchanged (still streamed) unless it reports itself dead
     st = upload_all();
     if (st != SLP_OK) return st;
   } else {
-    int n_stage = h->cfg.staging_slots == 0 ? h->E : std::min(h->cfg.staging_slots, h->E);
+    const int En = h->e1 - h->e0;
+    int n_stage = h->cfg.staging_slots == 0 ? En : std::min(h->cfg.staging_slots, En);
     int epl = h->cfg.experts_per_launch;
-    if (epl == 0) epl = auto_epl(n_stage, h->E);
+    if (epl == 0) epl = auto_epl(n_stage, En);
     st = alloc_pool(h, n_stage, epl);
     if (st != SLP_OK) {
       // still resident; if the pool had to be rebuilt on the way back its experts are uploaded again
@@ -929,7 +956,46 @@ slp_status slp_moe_prefill(slp_moe_layer* h, const void* hidden_bf16, int32_t T,
       return fail(SLP_ERR_CUDA, "cudaEventQuery failed: %s", cudaGetErrorString(q));
     }
   }
+  if (h->e0 != 0 || h->e1 != h->E)
+    return fail(SLP_ERR_INVALID_ARG, "this handle owns experts [%d, %d) of %d: use slp_moe_prefill_partial and reduce the partial sums", h->e0, h->e1, h->E);
   return prefill_impl(h, hidden_bf16, T, out_bf16, s);
+}
+
+slp_status slp_moe_prefill_partial(slp_moe_layer* h, const void* hidden_bf16, int32_t T, float* partial_f32, int32_t sh_t0, int32_t sh_t1,
+                                   void* cuda_stream) {
+  if (!h) return fail(SLP_ERR_INVALID_ARG, "NULL handle");
+  if (T < 0 || T > h->Tm) return fail(SLP_ERR_INVALID_ARG, "T = %d outside 0..max_tokens (%d)", T, h->Tm);
+  if (T == 0) return SLP_OK;
+  if (!hidden_bf16 || !partial_f32) return fail(SLP_ERR_INVALID_ARG, "NULL hidden/partial");
+  if (sh_t0 < 0 || sh_t1 < sh_t0 || sh_t1 > T) return fail(SLP_ERR_INVALID_ARG, "shared token range [%d, %d) outside 0..%d", sh_t0, sh_t1, T);
+  CU_TRY(cudaSetDevice(h->cfg.device));
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  if (h->dead) return fail(SLP_ERR_OOM, "handle lost its expert pool in an earlier failed residency switch; destroy it");
+  if (h->in_flight) {
+    cudaError_t q = cudaEventQuery(h->ev_done);
+    if (q == cudaSuccess) {
+      h->in_flight = false;
+      slp_status ke = check_kernel_error(h);
+      if (ke != SLP_OK) return ke;
+    } else if (q == cudaErrorNotReady) {
+      if (s != h->last_stream) return fail(SLP_ERR_BUSY, "a call is still in flight on another stream");
+    } else {
+      return fail(SLP_ERR_CUDA, "cudaEventQuery failed: %s", cudaGetErrorString(q));
+    }
+  }
+  return prefill_impl(h, hidden_bf16, T, partial_f32, s, true, sh_t0, sh_t1);
+}
+
+slp_status slp_moe_finalize_partial(int32_t device, const float* sum_f32, size_t n_elems, void* out_bf16, void* cuda_stream) {
+  if (!sum_f32 || !out_bf16) return fail(SLP_ERR_INVALID_ARG, "NULL argument");
+  if (n_elems % 4) return fail(SLP_ERR_INVALID_ARG, "n_elems must be a multiple of 4");
+  if (n_elems == 0) return SLP_OK;
+  CU_TRY(cudaSetDevice(device));
+  const size_t n4 = n_elems / 4;
+  const int blocks = static_cast<int>(std::min<size_t>((n4 + 255) / 256, 148 * 16));
+  slp::partial_to_bf16_kernel<<<blocks, 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(sum_f32, static_cast<__nv_bfloat16*>(out_bf16), n4);
+  CU_TRY(cudaGetLastError());
+  return SLP_OK;
 }
 
 slp_status slp_moe_prefill_host(slp_moe_layer* h, const void* hidden_host, int32_t T, void* out_host) {
@@ -937,6 +1003,7 @@ slp_status slp_moe_prefill_host(slp_moe_layer* h, const void* hidden_host, int32
   if (T < 0 || T > h->Tm) return fail(SLP_ERR_INVALID_ARG, "T = %d outside 0..max_tokens (%d)", T, h->Tm);
   if (T == 0) return SLP_OK;
   if (!hidden_host || !out_host) return fail(SLP_ERR_INVALID_ARG, "NULL hidden/out");
+  if (h->e0 != 0 || h->e1 != h->E) return fail(SLP_ERR_INVALID_ARG, "expert-sharded handle: use slp_moe_prefill_partial");
   CU_TRY(cudaSetDevice(h->cfg.device));
   if (h->dead) return fail(SLP_ERR_OOM, "handle lost its expert pool in an earlier failed residency switch; destroy it");
   slp_status st = wait_idle(h);
@@ -1083,8 +1150,14 @@ slp_status slp_moe_get_stats(slp_moe_layer* h, slp_moe_stats* stats) {
       h->stats.ms_gateup_sum += a;
       h->stats.ms_down_sum += b;
     }
-    unsigned long long clk[4] = {0, 0, 0, 0};
+    unsigned long long clk[16] = {};
     CU_TRY(cudaMemcpy(clk, h->d_clk, sizeof clk, cudaMemcpyDeviceToHost));
+#ifdef SLP_PROF
+    for (int m = 0; m < 2; ++m)
+      if (clk[7 + 4 * m])
+        fprintf(stderr, "[slp prof] mode %d: tiles/CTA-warp0 %llu, per tile: next-item %.0f, first-wait %.0f, K loop %.0f, epilogue %.0f cycles\n", m,
+                clk[7 + 4 * m], double(clk[12 + m]) / clk[7 + 4 * m], double(clk[4 + 4 * m]) / clk[7 + 4 * m], double(clk[5 + 4 * m]) / clk[7 + 4 * m], double(clk[6 + 4 * m]) / clk[7 + 4 * m]);
+#endif
     h->stats.sm_mhz_gateup = clk[1] ? static_cast<float>(1e3 * static_cast<double>(clk[0]) / static_cast<double>(clk[1])) : 0.f;
     h->stats.sm_mhz_down = clk[3] ? static_cast<float>(1e3 * static_cast<double>(clk[2]) / static_cast<double>(clk[3])) : 0.f;
     int32_t ts[1] = {0};

@@ -57,6 +57,9 @@ CONFIGS = [
     LayerConfig("cfg2_dsv3_T32768", 32768, 7168, 256, 8, 8, 4, 2048, 1, "sigmoid_bias", True, 2.5, 1, "normal", "streamed"),
     LayerConfig("cfg3_dsv3_zipf_T16384", 16384, 7168, 256, 8, 8, 4, 2048, 1, "sigmoid_bias", True, 2.5, 2, "zipf", "streamed"),
     LayerConfig("cfg4_softmax128_T8192", 8192, 4096, 128, 8, 1, 1, 1536, 0, "softmax", True, 1.0, 3, "none", "resident"),
+    # not a BASELINE config: the 384-expert Kimi-K2-shaped layer the paper also serves (16.9 GB of
+    # routed FP8 weights per layer): top-8 of 384, no expert groups, one shared expert.
+    LayerConfig("cfg5_k2_T4096", 4096, 7168, 384, 8, 1, 1, 2048, 1, "sigmoid_bias", True, 2.827, 4, "normal", "streamed"),
 ]
 
 _TENSOR_IDS = dict(hidden=1, router_w=2, bias=3, gate=4, up=5, down=6,
@@ -140,7 +143,7 @@ def _make_matrix(cfg, tensor, index, N, K, device):
     return quantize_weight_128x128(w)
 
 
-def make_weights(cfg, device="cpu", pin=False, experts=None):
+def make_weights(cfg, device="cpu", pin=False, experts=None, shard=None):
     """All layer weights as HOST tensors (pinned if `pin`), generated on `device`.
 
     Returns a dict of torch tensors:
@@ -150,8 +153,15 @@ def make_weights(cfg, device="cpu", pin=False, experts=None):
       shared_* (same shapes without the E axis) | None.
     `experts`: optional iterable restricting which experts are generated (others left zero);
     used by sampled full-size checks to save time.
+    `shard` = (e0, e1): allocate and generate only experts e0 .. e1 - 1 (an expert-parallel rank's share,
+    same bytes as the full layer's); the per-expert tensors then have e1 - e0 entries and the dict carries
+    "expert_offset" = e0.
     """
     E, H, I = cfg.E, cfg.H, cfg.I
+    e_off = 0
+    if shard is not None:
+        e_off, E = shard[0], shard[1] - shard[0]
+        experts = None
 
     def host(shape, dtype):
         return torch.empty(shape, dtype=dtype, pin_memory=pin)
@@ -169,9 +179,11 @@ def make_weights(cfg, device="cpu", pin=False, experts=None):
             out[key].zero_()
         for key in ("gate_s", "up_s", "down_s"):
             out[key].fill_(1.0)
+    if shard is not None:
+        out["expert_offset"] = e_off
     for e in todo:
         for name, N, K in (("gate", I, H), ("up", I, H), ("down", H, I)):
-            q, s = _make_matrix(cfg, name, e, N, K, device)
+            q, s = _make_matrix(cfg, name, e_off + e, N, K, device)
             out[name + "_q"][e].copy_(q)
             out[name + "_s"][e].copy_(s)
     for name, N, K in (("shared_gate", I, H), ("shared_up", I, H), ("shared_down", H, I)):
@@ -189,7 +201,7 @@ def make_weights(cfg, device="cpu", pin=False, experts=None):
 
 def weights_as_numpy(weights):
     """Zero-copy numpy views of `make_weights` output, in the mapping the oracle takes."""
-    return {k: (None if v is None else v.numpy()) for k, v in weights.items()}
+    return {k: (v if v is None or isinstance(v, int) else v.numpy()) for k, v in weights.items()}
 
 
 def hidden_as_bits(hidden):

@@ -31,8 +31,8 @@ def test_exports_every_declared_symbol(built):
 
 
 def test_struct_sizes_match_header(built):
-    # 18 four-byte fields / 14 pointers / see header
-    assert ctypes.sizeof(binding._Cfg) == 18 * 4
+    # 20 four-byte fields / 14 pointers / see header
+    assert ctypes.sizeof(binding._Cfg) == 20 * 4
     assert ctypes.sizeof(binding._HostWeights) == 14 * 8
     assert ctypes.sizeof(binding.Stats) == 96  # 80 + sm_mhz_gateup, sm_mhz_down + h2d_copies, reserved
 
