@@ -128,7 +128,10 @@ typedef struct {
   float sm_mhz_gateup;        /* average SM clock during the gate/up launches (clock64 / globaltimer of CTA 0) */
   float sm_mhz_down;          /* same for the down launches */
   int32_t h2d_copies;         /* cudaMemcpyAsync calls the streaming engine issued (consecutive experts merge) */
-  int32_t reserved;
+  int32_t experts_from_prefetch; /* experts of this call whose weights an earlier call had already prefetched (stacks) */
+  int32_t experts_prefetched; /* experts of the NEXT layer whose copies this call enqueued ahead (stacks) */
+  int32_t layer;              /* layer of the stack the call ran */
+  int64_t bytes_prefetched;   /* host -> HBM bytes of those prefetch copies (not part of bytes_copied) */
 } slp_moe_stats;
 
 /* What create would allocate and how prefill would launch for a configuration (host arithmetic only). */
@@ -167,6 +170,26 @@ typedef enum {
  * tensors, allocates workspace for cfg->max_tokens and the expert slots.  Starts in SLP_STREAMED.
  * Errors: INVALID_ARG (NULL / bad struct_size), UNSUPPORTED_SHAPE, NOT_PINNED, OOM, CUDA. */
 slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weights* w, slp_moe_layer** out);
+
+/* Multi-layer handle (Fig. 5: the loader walks the modules of successive layers while the model
+ * thread executes them; "the experts ring buffer is shared across layers").  n_layers weight sets of the same shape
+ * share ONE ring of expert slots, one workspace and one copy stream: the HBM cost of the streamed experts is
+ * staging_slots slots however many layers there are, and no cudaMalloc / cudaFree happens after create.
+ * `w` points to n_layers slp_moe_host_weights.  Router weights, biases, block scales and shared experts of all layers
+ * are uploaded at create and stay resident.  slp_moe_layer_create is the n_layers == 1 case; every call that takes
+ * a handle works on a stack (the single-layer calls address layer 0).  Resident mode needs n_layers == 1. */
+slp_status slp_moe_stack_create(const slp_moe_cfg* cfg, int32_t n_layers, const slp_moe_host_weights* w, slp_moe_layer** out);
+
+/* slp_moe_prefill on layer `layer` of a stack.  After enqueueing the layer's own work the loader keeps going: the
+ * copies of layer (layer + 1) % n_layers are enqueued on the copy stream, each waiting only for the OFF event of
+ * the ring slot it overwrites, so the next layer's experts stream in while this layer still computes and the next
+ * call finds them loaded (or loading) instead of starting its weight pass from scratch.  n_layers == 1: no
+ * prefetch.  Prefetched groups are always copied whole (routing of the next layer is not known yet). */
+slp_status slp_moe_stack_prefill(slp_moe_layer* h, int32_t layer, const void* hidden_bf16, int32_t T, void* out_bf16, void* cuda_stream);
+
+/* Explicit loader run-ahead: enqueue the copies of `layer` now (as many launch groups as the ring has slots that
+ * hold no unconsumed prefetch).  Returns immediately; a later slp_moe_stack_prefill(layer) consumes them. */
+slp_status slp_moe_stack_prefetch(slp_moe_layer* h, int32_t layer);
 
 /* Validates cfg exactly as create does and fills *plan; needs no GPU and allocates nothing.
  * Errors: INVALID_ARG, UNSUPPORTED_SHAPE (same messages as create). */

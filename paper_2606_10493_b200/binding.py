@@ -17,6 +17,7 @@ EXPORTED_SYMBOLS = [
     "slp_moe_debug_quant_hidden", "slp_moe_debug_buffer", "slp_moe_get_stats",
     "slp_measure_h2d", "slp_version", "slp_moe_query_plan", "slp_moe_debug_buffer_range",
     "slp_moe_prefill_partial", "slp_moe_finalize_partial",
+    "slp_moe_stack_create", "slp_moe_stack_prefill", "slp_moe_stack_prefetch",
 ]
 
 SLP_STREAMED, SLP_RESIDENT = 0, 1
@@ -59,7 +60,8 @@ class Stats(C.Structure):
                 ("gemm_launches", C.c_int32), ("kernel_launches", C.c_int32), ("m_tiles", C.c_int32),
                 ("timed_gemm_pairs", C.c_int32), ("ms_gateup_sum", C.c_float), ("ms_down_sum", C.c_float),
                 ("sm_mhz_gateup", C.c_float), ("sm_mhz_down", C.c_float),
-                ("h2d_copies", C.c_int32), ("reserved", C.c_int32)]
+                ("h2d_copies", C.c_int32), ("experts_from_prefetch", C.c_int32), ("experts_prefetched", C.c_int32),
+                ("layer", C.c_int32), ("bytes_prefetched", C.c_int64)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_ if n != "struct_size"}
@@ -81,6 +83,9 @@ def lib():
         L.slp_last_error.restype = C.c_char_p
         L.slp_version.restype = C.c_char_p
         L.slp_moe_layer_create.argtypes = [C.POINTER(_Cfg), C.POINTER(_HostWeights), C.POINTER(C.c_void_p)]
+        L.slp_moe_stack_create.argtypes = [C.POINTER(_Cfg), C.c_int32, C.POINTER(_HostWeights), C.POINTER(C.c_void_p)]
+        L.slp_moe_stack_prefill.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
+        L.slp_moe_stack_prefetch.argtypes = [C.c_void_p, C.c_int32]
         L.slp_moe_set_residency.argtypes = [C.c_void_p, C.c_int]
         L.slp_moe_prefill.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
         L.slp_moe_prefill_partial.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p]
@@ -184,24 +189,29 @@ class SlpMoeLayer:
         c = _make_cfg(cfg, max_tokens=self.max_tokens, device=device, staging_slots=staging_slots,
                       experts_per_launch=experts_per_launch, skip_empty_experts=skip_empty_experts,
                       require_pinned=require_pinned, expert_range=self.expert_range)
-        w = weights
-        off = w.get("expert_offset", 0)
-        self._arrays = {k: _ptr_array(w[k], cfg.E, off) for k in ("gate_q", "gate_s", "up_q", "up_s", "down_q", "down_s")}
+        layers = list(weights) if isinstance(weights, (list, tuple)) else [weights]   # a list = a multi-layer stack
+        self.n_layers = len(layers)
+        self._arrays = []
+        hws = (_HostWeights * self.n_layers)()
 
         def p(t):
             return None if t is None else t.data_ptr()
 
-        hw = _HostWeights(router_w=p(w["router_w"]), router_bias=p(w["router_bias"]),
-                          shared_gate_q=p(w["shared_gate_q"]), shared_gate_s=p(w["shared_gate_s"]),
-                          shared_up_q=p(w["shared_up_q"]), shared_up_s=p(w["shared_up_s"]),
-                          shared_down_q=p(w["shared_down_q"]), shared_down_s=p(w["shared_down_s"]))
-        for k, arr in self._arrays.items():
-            setattr(hw, k, C.cast(arr, C.POINTER(C.c_void_p)))
+        for l, w in enumerate(layers):
+            off = w.get("expert_offset", 0)
+            arrays = {k: _ptr_array(w[k], cfg.E, off) for k in ("gate_q", "gate_s", "up_q", "up_s", "down_q", "down_s")}
+            self._arrays.append(arrays)
+            hw = hws[l]
+            hw.router_w, hw.router_bias = p(w["router_w"]), p(w["router_bias"])
+            for name in ("shared_gate_q", "shared_gate_s", "shared_up_q", "shared_up_s", "shared_down_q", "shared_down_s"):
+                setattr(hw, name, p(w[name]))
+            for k, arr in arrays.items():
+                setattr(hw, k, C.cast(arr, C.POINTER(C.c_void_p)))
         saved = os.environ.get("SLP_TRIAGE")
         if triage is not None:
             os.environ["SLP_TRIAGE"] = triage
         try:
-            _check(lib().slp_moe_layer_create(C.byref(c), C.byref(hw), C.byref(self._h)))
+            _check(lib().slp_moe_stack_create(C.byref(c), self.n_layers, hws, C.byref(self._h)))
         finally:
             if triage is not None:
                 if saved is None:
@@ -214,15 +224,20 @@ class SlpMoeLayer:
         r = {"streamed": SLP_STREAMED, "resident": SLP_RESIDENT}[mode]
         _check(lib().slp_moe_set_residency(self._h, r))
 
-    def prefill(self, hidden, out=None, stream=None):
-        """hidden: CUDA bf16 [T, H] tensor.  Asynchronous on `stream` (default: current)."""
+    def prefill(self, hidden, out=None, stream=None, layer=0):
+        """hidden: CUDA bf16 [T, H] tensor.  Asynchronous on `stream` (default: current).  `layer`: which layer of
+        a multi-layer stack (slp_moe_stack_prefill; the next layer's experts are prefetched behind it)."""
         import torch
         assert hidden.is_cuda and hidden.dtype == torch.bfloat16 and hidden.is_contiguous()
         if out is None:
             out = torch.empty_like(hidden)
         s = torch.cuda.current_stream(hidden.device) if stream is None else stream
-        _check(lib().slp_moe_prefill(self._h, hidden.data_ptr(), hidden.shape[0], out.data_ptr(), s.cuda_stream))
+        _check(lib().slp_moe_stack_prefill(self._h, layer, hidden.data_ptr(), hidden.shape[0], out.data_ptr(), s.cuda_stream))
         return out
+
+    def prefetch(self, layer):
+        """slp_moe_stack_prefetch: let the loader run ahead with `layer`'s expert copies."""
+        _check(lib().slp_moe_stack_prefetch(self._h, layer))
 
     def prefill_partial(self, hidden_all, partial=None, shared_tokens=(0, 0), stream=None):
         """SmallEP: hidden_all = the all-gathered CUDA bf16 [T, H] hidden states; returns the fp32 [T, H] partial

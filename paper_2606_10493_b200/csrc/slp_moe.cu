@@ -13,6 +13,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <map>
 #include <mutex>
 #include <new>
 #include <string>
@@ -162,11 +163,31 @@ slp_status validate_cfg(const slp_moe_cfg* cfg, int* n_stage_out, int* epl_out) 
 
 }  // namespace
 
+// Everything that belongs to ONE layer of a stack: host pointers and the small resident tensors.  The handle
+// keeps the set of the layer it is working on in its own fields of the same names (select_layer).
+struct LayerW {
+  slp_moe_host_weights hw{};
+  std::vector<const uint8_t*> gate_q, up_q, down_q;
+  uint16_t* d_router_hl = nullptr;
+  CUtensorMap tm_rw{};
+  float *d_router_w = nullptr, *d_bias = nullptr, *d_gate_s = nullptr, *d_up_s = nullptr, *d_down_s = nullptr;
+  uint8_t* d_shpool = nullptr;  // [3][I*H] shared expert of layers > 0 (layer 0's sits in slot 0 of the ring pool)
+  CUtensorMap tm_shgu{}, tm_shd{};
+};
+
 struct slp_moe_layer {
   slp_moe_cfg cfg{};
   Triage triage{};
+  std::vector<LayerW> layers;  // n_layers weight sets sharing one ring, one workspace
+  int cur_layer = -1;
+  // ring occupancy, per ring group: which (layer, first expert) was loaded into it last, and whether that load
+  // was a prefetch nobody has consumed yet (the loader running ahead of the model thread)
+  std::vector<int> occ_layer, occ_e0;
+  std::vector<char> occ_prefetched;
   slp_moe_host_weights hw{};
   std::vector<const uint8_t*> gate_q, up_q, down_q;
+  uint8_t* d_shpool = nullptr;
+  CUtensorMap tm_shgu{}, tm_shd{};
   std::vector<void*> registered;  // host ranges pinned by create
   int H = 0, E = 0, k = 0, I = 0, Tm = 0;
   int e0 = 0, e1 = 0;  // owned routed experts [e0, e1) (SmallEP); the whole layer on one GPU
@@ -222,6 +243,27 @@ namespace {
 
 using L = slp_moe_layer;
 
+void select_layer(L* h, int l) {
+  if (h->cur_layer == l) return;
+  const LayerW& w = h->layers[l];
+  h->hw = w.hw;
+  h->gate_q = w.gate_q; h->up_q = w.up_q; h->down_q = w.down_q;
+  h->d_router_hl = w.d_router_hl; h->tm_rw = w.tm_rw;
+  h->d_router_w = w.d_router_w; h->d_bias = w.d_bias;
+  h->d_gate_s = w.d_gate_s; h->d_up_s = w.d_up_s; h->d_down_s = w.d_down_s;
+  h->d_shpool = w.d_shpool; h->tm_shgu = w.tm_shgu; h->tm_shd = w.tm_shd;
+  h->cur_layer = l;
+}
+void stash_layer(L* h, int l) {  // the inverse, used while a layer's tensors are being created
+  LayerW& w = h->layers[l];
+  w.hw = h->hw;
+  w.gate_q = h->gate_q; w.up_q = h->up_q; w.down_q = h->down_q;
+  w.d_router_hl = h->d_router_hl; w.tm_rw = h->tm_rw;
+  w.d_router_w = h->d_router_w; w.d_bias = h->d_bias;
+  w.d_gate_s = h->d_gate_s; w.d_up_s = h->d_up_s; w.d_down_s = h->d_down_s;
+  w.d_shpool = h->d_shpool; w.tm_shgu = h->tm_shgu; w.tm_shd = h->tm_shd;
+}
+
 struct Pool {
   uint8_t* d_pool = nullptr;
   std::vector<cudaEvent_t> ev_ready, ev_free;
@@ -257,9 +299,10 @@ slp_status build_pool(L* h, int n_stage, int epl, Pool* p) {
   // ~4 us gap between back-to-back 14.7 MB copies is 1.5 % of the link time (profiles/r1_h2d_chunks.md).
   const size_t S = static_cast<size_t>(1 + n_stage);
   if (h->cfg.n_shared) {
-    CU_TRY(cudaMemcpy(p->d_pool, h->hw.shared_gate_q, IH, cudaMemcpyHostToDevice));
-    CU_TRY(cudaMemcpy(p->d_pool + S * IH, h->hw.shared_up_q, IH, cudaMemcpyHostToDevice));
-    CU_TRY(cudaMemcpy(p->d_pool + 2 * S * IH, h->hw.shared_down_q, IH, cudaMemcpyHostToDevice));
+    const slp_moe_host_weights& w0 = h->layers[0].hw;  // slot 0 = the shared expert of layer 0 (resident)
+    CU_TRY(cudaMemcpy(p->d_pool, w0.shared_gate_q, IH, cudaMemcpyHostToDevice));
+    CU_TRY(cudaMemcpy(p->d_pool + S * IH, w0.shared_up_q, IH, cudaMemcpyHostToDevice));
+    CU_TRY(cudaMemcpy(p->d_pool + 2 * S * IH, w0.shared_down_q, IH, cudaMemcpyHostToDevice));
   } else {
     for (int kind = 0; kind < 3; ++kind) CU_TRY(cudaMemset(p->d_pool + kind * S * IH, 0, IH));
   }
@@ -306,6 +349,9 @@ slp_status alloc_pool(L* h, int n_stage, int epl) {
         h->tm_wgu = back.tm_wgu;
         h->tm_wd = back.tm_wd;
         h->free_recorded.assign(h->ev_ready.size(), 0);
+        h->occ_layer.assign(h->ev_ready.size(), -1);
+        h->occ_e0.assign(h->ev_ready.size(), -1);
+        h->occ_prefetched.assign(h->ev_ready.size(), 0);
         h->pool_needs_upload = true;  // resident experts were lost with the old pool
       } else {
         release_pool(&back);
@@ -325,9 +371,28 @@ slp_status alloc_pool(L* h, int n_stage, int epl) {
   h->tm_wgu = fresh.tm_wgu;
   h->tm_wd = fresh.tm_wd;
   h->free_recorded.assign(h->ev_ready.size(), 0);
+  h->occ_layer.assign(h->ev_ready.size(), -1);
+  h->occ_e0.assign(h->ev_ready.size(), -1);
+  h->occ_prefetched.assign(h->ev_ready.size(), 0);
   h->n_stage = n_stage;
   h->epl = epl;
   return SLP_OK;
+}
+
+// Host ranges this library registered with cudaHostRegister, process wide, with a reference count: two handles may
+// borrow the SAME host weight copy (prefill and decode share one resident DRAM copy, zero-copy), and
+// the range must stay page-locked until the last of them is destroyed.
+std::mutex g_reg_mutex;
+std::map<void*, int> g_registered;
+
+void unregister_host_range(void* p) {
+  std::lock_guard<std::mutex> lock(g_reg_mutex);
+  auto it = g_registered.find(p);
+  if (it == g_registered.end()) return;
+  if (--it->second == 0) {
+    cudaHostUnregister(p);
+    g_registered.erase(it);
+  }
 }
 
 // true if [p, p + bytes) is page-locked host memory as far as the runtime can tell (first and last byte)
@@ -352,6 +417,15 @@ slp_status pin_range(L* h, const void* p, size_t bytes, const char* what) {
   if (e == cudaSuccess && attr.type == cudaMemoryTypeDevice)
     return fail(SLP_ERR_INVALID_ARG, "%s is a device pointer; host weights are expected", what);
   cudaGetLastError();
+  {
+    std::lock_guard<std::mutex> lock(g_reg_mutex);
+    auto it = g_registered.find(const_cast<void*>(p));
+    if (it != g_registered.end()) {  // registered by another handle of this process: share it
+      ++it->second;
+      h->registered.push_back(const_cast<void*>(p));
+      return SLP_OK;
+    }
+  }
   if (range_is_pinned(p, bytes)) return SLP_OK;
   if (h->cfg.require_pinned) return fail(SLP_ERR_NOT_PINNED, "%s is pageable host memory and require_pinned is set", what);
   e = cudaHostRegister(const_cast<void*>(p), bytes, cudaHostRegisterDefault);
@@ -364,6 +438,10 @@ slp_status pin_range(L* h, const void* p, size_t bytes, const char* what) {
                                     "register the enclosing allocation once or pass pinned memory", what);
   }
   if (e != cudaSuccess) return fail(SLP_ERR_NOT_PINNED, "cudaHostRegister(%s, %zu bytes) failed: %s", what, bytes, cudaGetErrorString(e));
+  {
+    std::lock_guard<std::mutex> lock(g_reg_mutex);
+    g_registered[const_cast<void*>(p)] = 1;
+  }
   h->registered.push_back(const_cast<void*>(p));
   return SLP_OK;
 }
@@ -388,6 +466,7 @@ slp_status check_kernel_error(L* h) {
 
 slp::GemmArgs gemm_args(L* h, int mode, int e_begin, int e_end, int T) {
   slp::GemmArgs g{};
+  const bool sh_own_pool = e_begin == h->E && h->d_shpool != nullptr;  // shared expert of a layer > 0
   g.tile_expert = h->d_tile_expert;
   g.tile_start = h->d_tile_start;
   g.row_start = h->d_row_start;
@@ -402,11 +481,11 @@ slp::GemmArgs gemm_args(L* h, int mode, int e_begin, int e_end, int T) {
   g.e_own0 = h->e0;
   g.shared_rows = h->sh_rows;
   g.n_stage = h->n_stage;
-  g.n_slots = 1 + h->n_stage;
+  g.n_slots = sh_own_pool ? 1 : 1 + h->n_stage;
   g.a_q = mode == 0 ? h->d_xq : h->d_hq;
   g.a_s = mode == 0 ? h->d_xs : h->d_hs;
   g.a_s_stride = mode == 0 ? h->xs_stride : h->hs_stride;
-  g.pool = h->d_pool;
+  g.pool = sh_own_pool ? h->d_shpool : h->d_pool;
   g.gate_s = h->d_gate_s;
   g.up_s = h->d_up_s;
   g.down_s = h->d_down_s;
@@ -435,6 +514,9 @@ slp_status launch_experts(L* h, cudaStream_t s, int e_begin, int e_end, int T, i
   } else {
     slp::GemmArgs g0 = gemm_args(h, 0, e_begin, e_end, T), g1 = gemm_args(h, 1, e_begin, e_end, T);
     const int nt0 = h->I / 128, nt1 = (h->H + 255) / 256;
+    const bool sh_own_pool = e_begin == h->E && h->d_shpool != nullptr;  // shared expert of a layer > 0: its own small pool
+    const CUtensorMap& tm_wgu = sh_own_pool ? h->tm_shgu : h->tm_wgu;
+    const CUtensorMap& tm_wd = sh_own_pool ? h->tm_shd : h->tm_wd;
     cudaEvent_t* ev = (h->ev_k_used + 3 <= static_cast<int>(h->ev_k.size())) ? &h->ev_k[h->ev_k_used] : nullptr;
     if (h->triage.gemm == kGemmTc) CU_TRY(cudaMemsetAsync(h->d_sched, 0, 2 * sizeof(int), s));  // work-item counters of the two launches below
     if (ev) cudaEventRecord(ev[0], s);
@@ -454,23 +536,23 @@ slp_status launch_experts(L* h, cudaStream_t s, int e_begin, int e_end, int T, i
       lc.attrs = attr;
       lc.numAttrs = 1;
       lc.gridDim = dim3(2 * std::max(1, std::min(n_cl, max_tiles * nt0)));
-      CU_TRY(cudaLaunchKernelEx(&lc, tc::gemm_tc_kernel<0, true>, h->tm_xq, h->tm_wgu, h->tm_y, g0));
+      CU_TRY(cudaLaunchKernelEx(&lc, tc::gemm_tc_kernel<0, true>, h->tm_xq, tm_wgu, h->tm_y, g0));
       if (ev) cudaEventRecord(ev[1], s);
       lc.gridDim = dim3(2 * std::max(1, std::min(n_cl, max_tiles * nt1)));
       lc.dynamicSmemBytes = tc::Cfg<1, true>::kSmemBytes;
-      CU_TRY(cudaLaunchKernelEx(&lc, tc::gemm_tc_kernel<1, true>, h->tm_hq, h->tm_wd, h->tm_y, g1));
+      CU_TRY(cudaLaunchKernelEx(&lc, tc::gemm_tc_kernel<1, true>, h->tm_hq, tm_wd, h->tm_y, g1));
     } else {
       const int grid0 = std::max(1, std::min(h->num_sms, max_tiles * nt0));
       const int grid1 = std::max(1, std::min(h->num_sms, max_tiles * nt1));
       namespace tc = slp::tc;
       if (h->triage.gemm == kGemmTc) {  // dynamic tile distribution (the product path); 3 = static round-robin
-        tc::gemm_tc_kernel<0, false, true><<<grid0, tc::kThreads, tc::Cfg<0, false>::kSmemBytes, s>>>(h->tm_xq, h->tm_wgu, h->tm_y, g0);
+        tc::gemm_tc_kernel<0, false, true><<<grid0, tc::kThreads, tc::Cfg<0, false>::kSmemBytes, s>>>(h->tm_xq, tm_wgu, h->tm_y, g0);
         if (ev) cudaEventRecord(ev[1], s);
-        tc::gemm_tc_kernel<1, false, true><<<grid1, tc::kThreads, tc::Cfg<1, false>::kSmemBytes, s>>>(h->tm_hq, h->tm_wd, h->tm_y, g1);
+        tc::gemm_tc_kernel<1, false, true><<<grid1, tc::kThreads, tc::Cfg<1, false>::kSmemBytes, s>>>(h->tm_hq, tm_wd, h->tm_y, g1);
       } else {
-        tc::gemm_tc_kernel<0, false><<<grid0, tc::kThreads, tc::Cfg<0, false>::kSmemBytes, s>>>(h->tm_xq, h->tm_wgu, h->tm_y, g0);
+        tc::gemm_tc_kernel<0, false><<<grid0, tc::kThreads, tc::Cfg<0, false>::kSmemBytes, s>>>(h->tm_xq, tm_wgu, h->tm_y, g0);
         if (ev) cudaEventRecord(ev[1], s);
-        tc::gemm_tc_kernel<1, false><<<grid1, tc::kThreads, tc::Cfg<1, false>::kSmemBytes, s>>>(h->tm_hq, h->tm_wd, h->tm_y, g1);
+        tc::gemm_tc_kernel<1, false><<<grid1, tc::kThreads, tc::Cfg<1, false>::kSmemBytes, s>>>(h->tm_hq, tm_wd, h->tm_y, g1);
       }
     }
     if (ev) {
@@ -515,8 +597,12 @@ slp_status copy_experts(L* h, int e0, int e1, const int32_t* counts /* NULL = al
 
 // `partial`: out is fp32 [T, H], the unrounded weighted sum over the owned experts (+ the shared expert for tokens
 // in [sh_t0, sh_t1)); otherwise out is bf16 [T, H] and the shared expert covers every token.
-slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t s, bool partial = false, int sh_t0 = 0, int sh_t1 = -1) {
+slp_status prefetch_layer(L* h, int l);
+
+slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t s, bool partial = false, int sh_t0 = 0, int sh_t1 = -1,
+                        int layer = 0) {
   const int E = h->E, k = h->k, H = h->H;
+  select_layer(h, layer);
   if (sh_t1 < 0) sh_t1 = T;
   if (h->cfg.n_shared == 0) sh_t0 = sh_t1 = 0;
   const bool shared = sh_t1 > sh_t0;
@@ -526,6 +612,7 @@ slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t
   h->stats.struct_size = sizeof(slp_moe_stats);
   h->stats.tokens = T;
   h->stats.residency = h->residency;
+  h->stats.layer = layer;
   h->stats_copy_valid = false;
   h->ev_k_used = 0;
   auto launched = [&](int n) { h->stats.kernel_launches += n; };
@@ -637,26 +724,53 @@ slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t
       }
       if (need == 0) {
         h->stats.experts_skipped += e1 - e0;
+        if (h->occ_prefetched[r] && h->occ_layer[r] == layer && h->occ_e0[r] == e0) h->occ_prefetched[r] = 0;  // loaded ahead, not needed after all
         continue;
       }
-      if (h->free_recorded[r]) CU_TRY(cudaStreamWaitEvent(h->copy_stream, h->ev_free[r], 0));  // OFF -> slot reusable
-      if (first_copy) {
-        CU_TRY(cudaEventRecord(h->ev_copy0, h->copy_stream));
-        first_copy = false;
+      // already loaded (or loading) by an earlier call's run-ahead?  then this call only waits for its ON event
+      const bool have = h->occ_prefetched[r] && h->occ_layer[r] == layer && h->occ_e0[r] == e0;
+      if (have) {
+        h->stats.experts_from_prefetch += e1 - e0;
+      } else {
+        if (h->free_recorded[r]) CU_TRY(cudaStreamWaitEvent(h->copy_stream, h->ev_free[r], 0));  // OFF -> slot reusable
+        if (first_copy) {
+          CU_TRY(cudaEventRecord(h->ev_copy0, h->copy_stream));
+          first_copy = false;
+        }
+        for (int e = e0; e < e1; ++e)
+          if (skip && h->h_counts[e] == 0) h->stats.experts_skipped += 1;
+        {
+          slp_status st = copy_experts(h, e0, e1, skip ? h->h_counts : nullptr);
+          if (st != SLP_OK) return st;
+        }
+        CU_TRY(cudaEventRecord(h->ev_ready[r], h->copy_stream));  // ON
+        h->occ_layer[r] = layer;
+        h->occ_e0[r] = e0;
       }
-      for (int e = e0; e < e1; ++e)
-        if (skip && h->h_counts[e] == 0) h->stats.experts_skipped += 1;
-      {
-        slp_status st = copy_experts(h, e0, e1, skip ? h->h_counts : nullptr);
-        if (st != SLP_OK) return st;
-      }
-      CU_TRY(cudaEventRecord(h->ev_ready[r], h->copy_stream));  // ON
+      h->occ_prefetched[r] = 0;
       CU_TRY(cudaStreamWaitEvent(s, h->ev_ready[r], 0));
       const int bound = skip ? rows_bound : std::min(routed_tiles_bound, (T * k) / 128 + (e1 - e0));
       slp_status st = launch_experts(h, s, e0, e1, T, std::max(1, bound));
       if (st != SLP_OK) return st;
       CU_TRY(cudaEventRecord(h->ev_free[r], s));  // OFF
       h->free_recorded[r] = 1;
+    }
+    // the loader keeps going with the next layer's modules (Fig. 5)
+    const int n_layers = static_cast<int>(h->layers.size());
+    if (n_layers > 1) {
+      const int64_t b0 = h->stats.bytes_copied;
+      const int32_t c0 = h->stats.experts_copied;
+      if (first_copy) {
+        CU_TRY(cudaEventRecord(h->ev_copy0, h->copy_stream));
+        first_copy = false;
+      }
+      slp_status st = prefetch_layer(h, (layer + 1) % n_layers);
+      if (st != SLP_OK) return st;
+      h->stats.bytes_prefetched = h->stats.bytes_copied - b0;   // accounted apart from this layer's own weight pass
+      h->stats.experts_prefetched = h->stats.experts_copied - c0;
+      h->stats.bytes_copied = b0;
+      h->stats.experts_copied = c0;
+      select_layer(h, layer);
     }
     if (!first_copy) {
       CU_TRY(cudaEventRecord(h->ev_copy1, h->copy_stream));
@@ -678,6 +792,28 @@ slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t
   return SLP_OK;
 }
 
+// Loader run-ahead: enqueue the copies of layer l's launch groups into the ring (one pass over the ring at most),
+// stopping at the first slot that still holds a prefetch nobody consumed.  Each copy waits for the OFF event of the
+// launch that last used its slot.  Leaves layer l selected.
+slp_status prefetch_layer(L* h, int l) {
+  if (h->residency != SLP_STREAMED) return SLP_OK;
+  select_layer(h, l);
+  const int epl = h->epl, n_ring = static_cast<int>(h->ev_ready.size());
+  int grp = 0;
+  for (int e0 = h->e0; e0 < h->e1 && grp < n_ring; e0 += epl, ++grp) {
+    const int e1 = std::min(h->e1, e0 + epl), r = grp % n_ring;
+    if (h->occ_prefetched[r]) break;
+    if (h->free_recorded[r]) CU_TRY(cudaStreamWaitEvent(h->copy_stream, h->ev_free[r], 0));
+    slp_status st = copy_experts(h, e0, e1, nullptr);
+    if (st != SLP_OK) return st;
+    CU_TRY(cudaEventRecord(h->ev_ready[r], h->copy_stream));
+    h->occ_layer[r] = l;
+    h->occ_e0[r] = e0;
+    h->occ_prefetched[r] = 1;
+  }
+  return SLP_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -686,7 +822,13 @@ const char* slp_last_error(void) { return g_last_error.c_str(); }
 const char* slp_version(void) { return "slpmoe 0.1 (sm_100a)"; }
 
 slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weights* w, slp_moe_layer** out) {
-  if (!cfg || !w || !out) return fail(SLP_ERR_INVALID_ARG, "NULL argument");
+  return slp_moe_stack_create(cfg, 1, w, out);
+}
+
+slp_status slp_moe_stack_create(const slp_moe_cfg* cfg, int32_t n_layers, const slp_moe_host_weights* w_all, slp_moe_layer** out) {
+  if (!cfg || !w_all || !out) return fail(SLP_ERR_INVALID_ARG, "NULL argument");
+  if (n_layers < 1 || n_layers > 4096) return fail(SLP_ERR_INVALID_ARG, "n_layers %d outside 1..4096", n_layers);
+  const slp_moe_host_weights* w = w_all;
   if (cfg->struct_size != sizeof(slp_moe_cfg)) return fail(SLP_ERR_INVALID_ARG, "cfg.struct_size %u != %zu", cfg->struct_size, sizeof(slp_moe_cfg));
   *out = nullptr;
   const int H = cfg->hidden, E = cfg->n_experts, k = cfg->top_k, I = cfg->moe_intermediate;
@@ -695,10 +837,13 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
     slp_status vst = validate_cfg(cfg, &n_stage, &epl);
     if (vst != SLP_OK) return vst;
   }
-  if (!w->router_w || !w->gate_q || !w->gate_s || !w->up_q || !w->up_s || !w->down_q || !w->down_s)
-    return fail(SLP_ERR_INVALID_ARG, "NULL weight pointer");
-  if (cfg->n_shared && (!w->shared_gate_q || !w->shared_gate_s || !w->shared_up_q || !w->shared_up_s || !w->shared_down_q || !w->shared_down_s))
-    return fail(SLP_ERR_INVALID_ARG, "n_shared == 1 but a shared weight pointer is NULL");
+  for (int l = 0; l < n_layers; ++l) {
+    const slp_moe_host_weights* wl = w_all + l;
+    if (!wl->router_w || !wl->gate_q || !wl->gate_s || !wl->up_q || !wl->up_s || !wl->down_q || !wl->down_s)
+      return fail(SLP_ERR_INVALID_ARG, "NULL weight pointer (layer %d)", l);
+    if (cfg->n_shared && (!wl->shared_gate_q || !wl->shared_gate_s || !wl->shared_up_q || !wl->shared_up_s || !wl->shared_down_q || !wl->shared_down_s))
+      return fail(SLP_ERR_INVALID_ARG, "n_shared == 1 but a shared weight pointer is NULL (layer %d)", l);
+  }
 
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
@@ -715,7 +860,7 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
   if (!h) return fail(SLP_ERR_OOM, "out of host memory");
   h->cfg = *cfg;
   h->triage = read_triage();
-  h->hw = *w;
+  h->layers.resize(n_layers);
   h->H = H; h->E = E; h->k = k; h->I = I; h->Tm = cfg->max_tokens;
   h->e0 = cfg->expert_end == 0 ? 0 : cfg->expert_begin;
   h->e1 = cfg->expert_end == 0 ? E : cfg->expert_end;
@@ -729,10 +874,6 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
   h->rows_max = Tpad + round_up(h->Tm * k + E * 127, 128);
   h->tiles_max = h->rows_max / 128 + 1;
   h->n_chunks_max = (h->Tm + slp::kChunkTokens - 1) / slp::kChunkTokens;
-  h->gate_q.assign(w->gate_q, w->gate_q + E);
-  h->up_q.assign(w->up_q, w->up_q + E);
-  h->down_q.assign(w->down_q, w->down_q + E);
-
   auto bail = [&](slp_status st) {
     std::string keep = g_last_error;
     slp_moe_layer_destroy(h);
@@ -752,8 +893,27 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
                        cudaGetErrorString(_e)));                                                                \
   } while (0)
 
-  // pin (or check) the streamed weights
   const size_t IH = static_cast<size_t>(I) * H;
+  CU_OR_BAIL(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
+  CU_OR_BAIL(cudaStreamCreateWithFlags(&h->own_stream, cudaStreamNonBlocking));
+  CU_OR_BAIL(cudaEventCreateWithFlags(&h->ev_done, cudaEventDisableTiming));
+  for (auto& e : h->ev_t) CU_OR_BAIL(cudaEventCreate(&e));
+  CU_OR_BAIL(cudaEventCreate(&h->ev_copy0));
+  CU_OR_BAIL(cudaEventCreate(&h->ev_copy1));
+  h->ev_k.resize(3 * (E + 2));
+  for (auto& e : h->ev_k) CU_OR_BAIL(cudaEventCreate(&e));
+
+  // ---- per layer: pin (or check) the streamed weights, upload router / bias / block scales / shared expert ----
+  CU_OR_BAIL(cudaFuncSetAttribute(slp::rtc::router_logits_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::rtc::kSmemBytes));
+  for (int l = 0; l < n_layers; ++l) {
+    w = w_all + l;
+    h->hw = *w;
+    h->gate_q.assign(w->gate_q, w->gate_q + E);
+    h->up_q.assign(w->up_q, w->up_q + E);
+    h->down_q.assign(w->down_q, w->down_q + E);
+    h->d_router_hl = nullptr; h->d_router_w = h->d_bias = h->d_gate_s = h->d_up_s = h->d_down_s = nullptr; h->d_shpool = nullptr;
+    h->cur_layer = l;
+    // (a failure below goes through bail -> destroy, which first stashes this half-built layer so that its tensors are freed)
   for (int e = h->e0; e < h->e1; ++e)
     if (!h->gate_q[e] || !h->up_q[e] || !h->down_q[e] || !w->gate_s[e] || !w->up_s[e] || !w->down_s[e])
       return bail(fail(SLP_ERR_INVALID_ARG, "NULL weight pointer for expert %d", e));
@@ -773,15 +933,6 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
     }
   }
 
-  CU_OR_BAIL(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
-  CU_OR_BAIL(cudaStreamCreateWithFlags(&h->own_stream, cudaStreamNonBlocking));
-  CU_OR_BAIL(cudaEventCreateWithFlags(&h->ev_done, cudaEventDisableTiming));
-  for (auto& e : h->ev_t) CU_OR_BAIL(cudaEventCreate(&e));
-  CU_OR_BAIL(cudaEventCreate(&h->ev_copy0));
-  CU_OR_BAIL(cudaEventCreate(&h->ev_copy1));
-  h->ev_k.resize(3 * (E + 2));
-  for (auto& e : h->ev_k) CU_OR_BAIL(cudaEventCreate(&e));
-
   // resident tensors: router, bias, all block scales (entry E = shared expert)
   const size_t sc_gu = static_cast<size_t>(h->kbI) * h->kbH, sc_d = static_cast<size_t>(h->kbH) * h->kbI;
   CU_OR_BAIL(cudaMalloc(&h->d_router_w, static_cast<size_t>(E) * H * sizeof(float)));
@@ -794,7 +945,6 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
     slp::rtc::split_router_w_kernel<<<h->num_sms * 4, 256>>>(h->d_router_w, h->d_router_hl, E, H, h->Erows);
     CU_OR_BAIL(cudaGetLastError());
     TRY_OR_BAIL(make_tmap_u8(&h->tm_rw, h->d_router_hl, static_cast<uint64_t>(H) * 2, static_cast<uint64_t>(2) * h->Erows));
-    CU_OR_BAIL(cudaFuncSetAttribute(slp::rtc::router_logits_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::rtc::kSmemBytes));
   }
   CU_OR_BAIL(cudaMalloc(&h->d_bias, E * sizeof(float)));
   if (w->router_bias) CU_OR_BAIL(cudaMemcpy(h->d_bias, w->router_bias, E * sizeof(float), cudaMemcpyHostToDevice));
@@ -812,6 +962,19 @@ slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weigh
     CU_OR_BAIL(cudaMemcpy(h->d_up_s + E * sc_gu, w->shared_up_s, sc_gu * sizeof(float), cudaMemcpyHostToDevice));
     CU_OR_BAIL(cudaMemcpy(h->d_down_s + E * sc_d, w->shared_down_s, sc_d * sizeof(float), cudaMemcpyHostToDevice));
   }
+
+    if (cfg->n_shared && l > 0) {  // layer 0's shared expert lives in slot 0 of the ring pool
+      CU_OR_BAIL(cudaMalloc(&h->d_shpool, 3 * IH));
+      CU_OR_BAIL(cudaMemcpy(h->d_shpool, w->shared_gate_q, IH, cudaMemcpyHostToDevice));
+      CU_OR_BAIL(cudaMemcpy(h->d_shpool + IH, w->shared_up_q, IH, cudaMemcpyHostToDevice));
+      CU_OR_BAIL(cudaMemcpy(h->d_shpool + 2 * IH, w->shared_down_q, IH, cudaMemcpyHostToDevice));
+      TRY_OR_BAIL(make_tmap_u8(&h->tm_shgu, h->d_shpool, h->H, static_cast<uint64_t>(3) * h->I, slp::tc::kBoxRows));
+      TRY_OR_BAIL(make_tmap_u8(&h->tm_shd, h->d_shpool, h->I, static_cast<uint64_t>(3) * h->H, slp::tc::kBoxRows));
+    }
+    stash_layer(h, l);
+  }
+  h->cur_layer = -1;
+  select_layer(h, 0);
 
   // workspace
   const size_t Tm = h->Tm, rows = h->rows_max;
@@ -914,6 +1077,9 @@ slp_status slp_moe_set_residency(slp_moe_layer* h, slp_residency r) {
     if (r == SLP_RESIDENT && h->pool_needs_upload) return upload_all();
     return SLP_OK;
   }
+  if (r == SLP_RESIDENT && h->layers.size() > 1)
+    return fail(SLP_ERR_UNSUPPORTED_SHAPE, "resident mode needs a single-layer handle (this stack has %zu layers sharing one ring)", h->layers.size());
+  select_layer(h, 0);
   if (r == SLP_RESIDENT) {
     st = alloc_pool(h, h->e1 - h->e0, h->e1 - h->e0);
     if (st != SLP_OK) return st;   // the handle is unchanged (still streamed) unless it reports itself dead
@@ -936,7 +1102,23 @@ slp_status slp_moe_set_residency(slp_moe_layer* h, slp_residency r) {
 }
 
 slp_status slp_moe_prefill(slp_moe_layer* h, const void* hidden_bf16, int32_t T, void* out_bf16, void* cuda_stream) {
+  return slp_moe_stack_prefill(h, 0, hidden_bf16, T, out_bf16, cuda_stream);
+}
+
+slp_status slp_moe_stack_prefetch(slp_moe_layer* h, int32_t layer) {
   if (!h) return fail(SLP_ERR_INVALID_ARG, "NULL handle");
+  if (layer < 0 || layer >= static_cast<int>(h->layers.size())) return fail(SLP_ERR_INVALID_ARG, "layer %d outside 0..%zu", layer, h->layers.size() - 1);
+  if (h->dead) return fail(SLP_ERR_OOM, "handle lost its expert pool in an earlier failed residency switch; destroy it");
+  CU_TRY(cudaSetDevice(h->cfg.device));
+  const slp_moe_stats keep = h->stats;   // a bare prefetch is not a call: it leaves the last call's statistics alone
+  slp_status st = prefetch_layer(h, layer);
+  h->stats = keep;
+  return st;
+}
+
+slp_status slp_moe_stack_prefill(slp_moe_layer* h, int32_t layer, const void* hidden_bf16, int32_t T, void* out_bf16, void* cuda_stream) {
+  if (!h) return fail(SLP_ERR_INVALID_ARG, "NULL handle");
+  if (layer < 0 || layer >= static_cast<int>(h->layers.size())) return fail(SLP_ERR_INVALID_ARG, "layer %d outside 0..%zu", layer, h->layers.size() - 1);
   if (T < 0 || T > h->Tm) return fail(SLP_ERR_INVALID_ARG, "T = %d outside 0..max_tokens (%d)", T, h->Tm);
   if (T == 0) return SLP_OK;
   if (!hidden_bf16 || !out_bf16) return fail(SLP_ERR_INVALID_ARG, "NULL hidden/out");
@@ -958,7 +1140,7 @@ slp_status slp_moe_prefill(slp_moe_layer* h, const void* hidden_bf16, int32_t T,
   }
   if (h->e0 != 0 || h->e1 != h->E)
     return fail(SLP_ERR_INVALID_ARG, "this handle owns experts [%d, %d) of %d: use slp_moe_prefill_partial and reduce the partial sums", h->e0, h->e1, h->E);
-  return prefill_impl(h, hidden_bf16, T, out_bf16, s);
+  return prefill_impl(h, hidden_bf16, T, out_bf16, s, false, 0, -1, layer);
 }
 
 slp_status slp_moe_prefill_partial(slp_moe_layer* h, const void* hidden_bf16, int32_t T, float* partial_f32, int32_t sh_t0, int32_t sh_t1,
@@ -1028,14 +1210,20 @@ slp_status slp_moe_layer_destroy(slp_moe_layer* h) {
   cudaSetDevice(h->cfg.device);
   cudaDeviceSynchronize();
   free_pool(h);
-  void* ptrs[] = {h->d_router_hl, h->d_router_w, h->d_bias, h->d_gate_s, h->d_up_s, h->d_down_s, h->d_logits, h->d_w, h->d_xs, h->d_hs, h->d_idx,
+  if (h->cur_layer >= 0 && h->cur_layer < static_cast<int>(h->layers.size())) stash_layer(h, h->cur_layer);
+  for (LayerW& w : h->layers) {
+    void* lp[] = {w.d_router_hl, w.d_router_w, w.d_bias, w.d_gate_s, w.d_up_s, w.d_down_s, w.d_shpool};
+    for (void* p : lp)
+      if (p) cudaFree(p);
+  }
+  void* ptrs[] = {h->d_logits, h->d_w, h->d_xs, h->d_hs, h->d_idx,
                   h->d_counts, h->d_chunk, h->d_row_start, h->d_tile_start, h->d_tile_expert, h->d_pair_start, h->d_pair_expert, h->d_tile_info, h->d_pos, h->d_row_token, h->d_xq,
                   h->d_hq, h->d_y, h->d_ys, h->d_err, h->d_clk, h->d_sched, h->d_e2e_in, h->d_e2e_out};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   if (h->h_counts) cudaFreeHost(h->h_counts);
   if (h->h_err) cudaFreeHost(h->h_err);
-  for (void* p : h->registered) cudaHostUnregister(p);
+  for (void* p : h->registered) unregister_host_range(p);
   if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
   if (h->own_stream) cudaStreamDestroy(h->own_stream);
   if (h->ev_done) cudaEventDestroy(h->ev_done);

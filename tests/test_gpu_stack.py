@@ -1,0 +1,162 @@
+"""Multi-layer stack with a cross-layer experts ring (Fig. 5) and one host weight copy shared by
+two handles, on reduced layers.  A stack's layer l must give exactly what a single-layer handle on
+the same weights gives (same kernels, same bytes: bitwise), while its expert copies are enqueued one layer ahead."""
+
+import ctypes
+
+import numpy as np
+import pytest
+import torch
+
+from oracle.acceptance import compare_routing, compare_output
+from paper_2606_10493_b200 import SlpMoeLayer, SlpError, inputs
+from test_gpu_parity import small_dsv3, problem
+
+pytestmark = pytest.mark.gpu
+
+N_LAYERS = 3
+
+
+@pytest.fixture(scope="module")
+def layers():
+    cfgs = [small_dsv3(name=f"stack_l{l}", T=700, seed=40 + l) for l in range(N_LAYERS)]
+    Ws = [inputs.make_weights(c, device="cpu", pin=True) for c in cfgs]
+    hidden = inputs.make_hidden(cfgs[0], device="cpu").cuda()
+    singles = []
+    for c, W in zip(cfgs, Ws):
+        one = SlpMoeLayer(c, W, device=0)
+        try:
+            singles.append(one.prefill(hidden).clone())
+            torch.cuda.synchronize()
+        finally:
+            one.close()
+    return cfgs, Ws, hidden, singles
+
+
+def test_stack_layers_equal_single_layer_handles_and_prefetch_accounting(layers):
+    cfgs, Ws, hidden, singles = layers
+    cfg = cfgs[0]
+    per_layer = cfg.E * 3 * cfg.I * cfg.H
+    stack = SlpMoeLayer(cfg, Ws, device=0)
+    try:
+        assert stack.n_layers == N_LAYERS
+        for rnd in range(2):
+            for l in range(N_LAYERS):
+                out = stack.prefill(hidden, layer=l).clone()
+                torch.cuda.synchronize()
+                st = stack.stats()
+                assert torch.equal(out.view(torch.int16), singles[l].view(torch.int16)), (rnd, l)
+                assert st["layer"] == l
+                first = rnd == 0 and l == 0
+                # the very first call loads its own experts; every later call finds them prefetched by its predecessor
+                assert st["experts_copied"] == (cfg.E if first else 0) and st["bytes_copied"] == (per_layer if first else 0)
+                assert st["experts_from_prefetch"] == (0 if first else cfg.E)
+                assert st["experts_prefetched"] == cfg.E and st["bytes_prefetched"] == per_layer   # next layer, wrapping to 0
+        with pytest.raises(SlpError) as ei:
+            stack.set_residency("resident")
+        assert ei.value.status == -2
+        with pytest.raises(SlpError):
+            stack.prefill(hidden, layer=N_LAYERS)
+    finally:
+        stack.close()
+
+
+def test_stack_out_of_order_and_explicit_prefetch(layers):
+    cfgs, Ws, hidden, singles = layers
+    cfg = cfgs[0]
+    stack = SlpMoeLayer(cfg, Ws, device=0)
+    try:
+        a = stack.prefill(hidden, layer=0).clone()            # prefetches layer 1 ...
+        b = stack.prefill(hidden, layer=2).clone()            # ... but layer 2 runs next: the prefetch is overwritten
+        torch.cuda.synchronize()
+        st = stack.stats()
+        assert st["experts_from_prefetch"] == 0 and st["experts_copied"] == cfg.E
+        stack.prefetch(1)                                     # explicit loader run-ahead (layer 0 is already prefetched: ring full)
+        c = stack.prefill(hidden, layer=1).clone()
+        torch.cuda.synchronize()
+        st1 = stack.stats()
+        d = stack.prefill(hidden, layer=0).clone()
+        torch.cuda.synchronize()
+    finally:
+        stack.close()
+    for got, l in ((a, 0), (b, 2), (c, 1), (d, 0)):
+        assert torch.equal(got.view(torch.int16), singles[l].view(torch.int16)), l
+    assert st1["experts_from_prefetch"] + st1["experts_copied"] == cfg.E
+
+
+@pytest.mark.parametrize("kw", [dict(staging_slots=8, experts_per_launch=4), dict(staging_slots=2, experts_per_launch=1),
+                                dict(staging_slots=16, experts_per_launch=8, skip_empty_experts=True)])
+def test_stack_with_a_ring_shorter_than_a_layer(layers, kw):
+    """Ring length below the number of experts of a layer (down to 2, ping-pong): only the first ring
+    pass of the next layer can be prefetched, the rest streams during the call."""
+    cfgs, Ws, hidden, singles = layers
+    cfg = cfgs[0]
+    stack = SlpMoeLayer(cfg, Ws, device=0, **kw)
+    try:
+        for l in (0, 1, 2, 0):
+            out = stack.prefill(hidden, layer=l).clone()
+            torch.cuda.synchronize()
+            st = stack.stats()
+            assert torch.equal(out.view(torch.int16), singles[l].view(torch.int16)), (kw, l)
+            assert st["experts_prefetched"] == kw["staging_slots"]
+            assert st["experts_from_prefetch"] + st["experts_copied"] + st["experts_skipped"] == cfg.E
+    finally:
+        stack.close()
+
+
+def test_stack_against_oracle(layers):
+    from oracle import moe_layer
+    cfgs, Ws, hidden, singles = layers
+    cfg = cfgs[1]
+    ref = moe_layer(inputs.hidden_as_bits(hidden), inputs.weights_as_numpy(Ws[1]), top_k=cfg.k, n_group=cfg.G, topk_group=cfg.Gk,
+                    scoring=cfg.scoring, norm_topk=cfg.norm_topk, routed_scale=cfg.routed_scale)
+    stack = SlpMoeLayer(cfg, Ws, device=0)
+    try:
+        stack.prefill(hidden, layer=0)
+        out = stack.prefill(hidden, layer=1).clone()
+        torch.cuda.synchronize()
+        idx, w, _ = stack.debug_routing(cfg.T)
+    finally:
+        stack.close()
+    r = compare_routing(idx, w, ref["route"])
+    o = compare_output(inputs.hidden_as_bits(out), ref["out_f64"], r["members_equal"])
+    assert r["passed"] and o["passed"], (r, o)
+
+
+def test_two_handles_share_one_pageable_host_copy():
+    """one resident DRAM copy of the weights serves two consumers.  Two handles borrow the same
+    PAGEABLE host tensors: the library page-locks each range once, counts its users, and keeps it locked until the
+    last handle goes away."""
+    cfg, _, hidden, ref = problem("mini_dsv3")
+    W = inputs.make_weights(cfg, device="cpu", pin=False)
+    x = hidden.cuda()
+    cudart = ctypes.CDLL("libcudart.so.12")
+    ptr, nbytes = W["gate_q"].data_ptr(), W["gate_q"].numel()
+
+    def still_registered():
+        rc = cudart.cudaHostRegister(ctypes.c_void_p(ptr), ctypes.c_size_t(nbytes), 0)
+        if rc == 0:                                    # it was NOT registered any more: undo and report
+            cudart.cudaHostUnregister(ctypes.c_void_p(ptr))
+            return False
+        cudart.cudaGetLastError()
+        return True
+
+    a = SlpMoeLayer(cfg, W, device=0)
+    b = SlpMoeLayer(cfg, W, device=0, staging_slots=4, experts_per_launch=2)
+    try:
+        oa = a.prefill(x).clone()
+        ob = b.prefill(x).clone()
+        torch.cuda.synchronize()
+        assert torch.equal(oa.view(torch.int16), ob.view(torch.int16))
+        a.close()
+        assert still_registered(), "destroying the first handle unpinned memory the second one still streams from"
+        ob2 = b.prefill(x).clone()
+        torch.cuda.synchronize()
+        assert torch.equal(ob2.view(torch.int16), oa.view(torch.int16))
+    finally:
+        a.close()
+        b.close()
+    assert not still_registered(), "the last handle must release the registration"
+    with pytest.raises(SlpError) as ei:
+        SlpMoeLayer(cfg, W, device=0, require_pinned=True)
+    assert ei.value.status == -5
