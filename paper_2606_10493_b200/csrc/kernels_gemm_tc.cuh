@@ -48,6 +48,7 @@
 namespace slp {
 namespace tc {
 
+
 constexpr int BM = 128, BN = 256, BK = 128, HN = 128;
 constexpr int kBoxRows = 64;  // rows per B TMA box
 constexpr int kEpiWarps = 8;
@@ -55,6 +56,7 @@ constexpr int kThreads = (kEpiWarps + 4) * 32;  // three warpgroups: 2 x promoti
 constexpr int kTmemCols = 512;
 constexpr int kMaxStages = 6;
 constexpr int kSchedDepth = 4;  // work items the scheduler warp may run ahead of the roles
+constexpr int kWsCap = 64;      // K blocks of weight scales a promotion warp keeps in shared memory (refilled beyond)
 
 // kPair = false: one CTA per tile, A tile (16 KB) + whole B tile (32 KB) per stage, 4 stages.
 // kPair = true:  a cluster of two CTAs issues one cta_group::2 MMA with M = 256 (two 128-row tiles
@@ -64,12 +66,15 @@ constexpr int kSchedDepth = 4;  // work items the scheduler warp may run ahead o
 template <int kMode, bool kPair> struct Cfg {
   // The down kernel trades one pipeline stage for a staging area that holds its whole fp16 Y tile
   // (64 KB): its tiles are only 16 K blocks long, so the epilogue must not wait on TMA-store read-out.
-  static constexpr int kStages = kPair ? (kMode == 1 ? 5 : 6) : (kMode == 1 ? 3 : 4);
+  static constexpr int kStages = kPair ? (kMode == 1 ? 4 : 6) : (kMode == 1 ? 3 : 4);
   static constexpr int kABytes = BM * BK;
   static constexpr int kBBytes = (kPair ? BN / 2 : BN) * BK;
   static constexpr int kStageBytes = kABytes + kBBytes;
-  static constexpr int kScratchBytes = kMode == 1 ? kEpiWarps * 8192 : 32768;  // mode 1: the whole fp16 Y tile (two 4 KB boxes per warp); mode 0: amax exchange only
-  static constexpr int kSmemBytes = kStages * kStageBytes + 1024 /*align*/ + 256 /*barriers*/ + kScratchBytes;
+  // mode 1: the whole fp16 Y tile (two 4 KB boxes per warp); mode 0: the amax exchange (2 KB); both: the per-warp
+  // weight-scale tables of the promotion loop (kWsCap float2 per warp)
+  static constexpr int kYBytes = kMode == 1 ? kEpiWarps * 8192 : 2048;
+  static constexpr int kScratchBytes = kYBytes + kEpiWarps * kWsCap * 8;
+  static constexpr int kSmemBytes = kStages * kStageBytes + 1024 /*align*/ + 512 /*barriers*/ + kScratchBytes;
   static_assert(kSmemBytes <= 232448, "shared memory budget");
 };
 
@@ -77,25 +82,30 @@ template <int kMode, bool kPair> struct Cfg {
 struct Shared {
   uint64_t full[kMaxStages];   // TMA -> MMA: stage landed (pair: lives in the leader CTA, fed by both CTAs' loads)
   uint64_t empty[kMaxStages];  // MMA -> TMA: stage consumed (pair: multicast commit to both CTAs)
-  uint64_t tmem_full[2];       // MMA -> promotion: K block partial complete in TMEM buffer b
-  uint64_t tmem_empty[2];      // promotion -> MMA: buffer b read out (pair: 2 x kEpiWarps arrivals at the leader)
+  uint64_t tmem_full[2][2];    // MMA -> promotion: columns [128 h, 128 h + 128) of the K block partial complete in TMEM buffer b: [b][h]
+  uint64_t tmem_empty[2][2];   // promotion -> MMA: that half of buffer b read out by its kEpiWarps / 2 warps (pair: both CTAs', at the leader)
   uint64_t sched_full[kSchedDepth];   // scheduler -> roles: work item published
   uint64_t sched_empty[kSchedDepth];  // roles -> scheduler: slot read by producer, MMA issuer and the promotion warps
-  int32_t sched_w[kSchedDepth];       // work item of each slot (-1 = no more work)
+  int4 sched_rec[kSchedDepth];        // tile record of each slot {expert (-1 = no more work), first row, valid rows, N tile}
   uint32_t tmem_base;
   int dead;
 };
-static_assert(sizeof(Shared) <= 256, "barrier block");
-constexpr uint32_t kOffFull = 0, kOffEmpty = 8 * kMaxStages, kOffTmemFull = 16 * kMaxStages, kOffTmemEmpty = 16 * kMaxStages + 16;
-constexpr uint32_t kOffSchedFull = kOffTmemEmpty + 16, kOffSchedEmpty = kOffSchedFull + 8 * kSchedDepth;
+static_assert(sizeof(Shared) <= 512, "barrier block");
+constexpr uint32_t kOffFull = 0, kOffEmpty = 8 * kMaxStages, kOffTmemFull = 16 * kMaxStages, kOffTmemEmpty = 16 * kMaxStages + 32;
+constexpr uint32_t kOffSchedFull = kOffTmemEmpty + 32, kOffSchedEmpty = kOffSchedFull + 8 * kSchedDepth;
 
-// silu(g) * u with the fast exponential and reciprocal (rel. error ~1e-6, three decades below the
-// e4m3 step that follows).
-__device__ __forceinline__ float silu_mul_fast(float g, float u) {
-  float t, r;
-  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(t) : "f"(g * -1.4426950408889634f));  // e^-g; overflow -> +inf -> r = 0
-  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(1.0f + t));
-  return g * r * u;
+// silu(g) * u for two elements with the fast exponential and ONE reciprocal (rel. error ~1e-6, three decades below
+// the e4m3 step that follows): 1 / a = b * rcp(a b), 1 / b = a * rcp(a b) with a = 1 + e^-g0, b = 1 + e^-g1.  The SFU
+// (16 results per clock per SM) bounds this epilogue, so three instead of four SFU operations per pair matter.
+// e^-g is clamped to 2^60 so that the product stays finite (silu(g) < 2^-54 there anyway).
+__device__ __forceinline__ void silu_mul_fast2(float& g0, float u0, float& g1, float u1) {
+  float t0, t1, r;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(t0) : "f"(g0 * -1.4426950408889634f));
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(t1) : "f"(g1 * -1.4426950408889634f));
+  const float a = 1.0f + fminf(t0, 0x1p60f), b = 1.0f + fminf(t1, 0x1p60f);
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a * b));
+  g0 = g0 * (r * b) * u0;
+  g1 = g1 * (r * a) * u1;
 }
 
 // p ? a : b as one SELP (keeps the scale bookkeeping of the K loop free of branches and copies).
@@ -152,7 +162,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < kStages; ++i) { ptx::mbar_init(&sh->full[i], 1); ptx::mbar_init(&sh->empty[i], 1); }
-    for (int i = 0; i < 2; ++i) { ptx::mbar_init(&sh->tmem_full[i], 1); ptx::mbar_init(&sh->tmem_empty[i], kPair ? 2 * kEpiWarps : kEpiWarps); }
+    for (int i = 0; i < 4; ++i) { ptx::mbar_init(&sh->tmem_full[i >> 1][i & 1], 1); ptx::mbar_init(&sh->tmem_empty[i >> 1][i & 1], kPair ? kEpiWarps : kEpiWarps / 2); }
     for (int i = 0; i < kSchedDepth; ++i) { ptx::mbar_init(&sh->sched_full[i], 1); ptx::mbar_init(&sh->sched_empty[i], 2 + kEpiWarps); }
     sh->dead = 0;
     ptx::fence_mbar_init();
@@ -194,17 +204,25 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
     return t;
   };
 
-  // Next work item of this CTA after `w` (its i-th), or -1.  Static order: w + gridDim.  kDyn (one-CTA
-  // kernel, the default; SLP_TRIAGE gemm=static selects the static order): items come from a global counter through a small shared-memory ring fed by an idle warp, so
-  // all CTAs stay inside a window of ~gridDim consecutive items and the B tiles they share stay in L2
-  // (profiles/r1_sched_ab.md).  Which CTA computes a tile does not change its result.
-  auto next_item = [&](int w, int i, bool whole_warp) -> int {
+  // Tile that follows this CTA's i-th one (e < 0: none).  Static order: item w + gridDim, record read from global
+  // memory.  kDyn (one-CTA kernel, the default; SLP_TRIAGE gemm=static selects the static order): items come from a
+  // global counter, so all CTAs stay inside a window of ~gridDim consecutive items and the B tiles they share stay in
+  // L2 (profiles/r1_sched_ab.md).  An otherwise idle warp takes the item AND reads its record, and publishes the
+  // record through a four-deep ring in shared memory: the roles pay one barrier wait and one 16-byte shared load per
+  // tile instead of a global-memory round trip (a record held in registers across the K loop was being spilled and
+  // cost the promotion warps ~650 cycles per tile).  Which CTA computes a tile does not change its result.
+  const uint32_t rec_a = bar_a + static_cast<uint32_t>(offsetof(Shared, sched_rec));
+  auto next_tile = [&](int& w, int i, bool whole_warp) -> Tile {
+    Tile t;
     if constexpr (kPair || !kDyn) {
       w += w_step;
+      if (w < total) t = fetch(w);
+      else t.e = -1;
     } else {
       const uint32_t slot = static_cast<uint32_t>(i) % kSchedDepth;
       ptx::mbar_wait_a(bar_a + kOffSchedFull + 8 * slot, (static_cast<uint32_t>(i) / kSchedDepth) & 1, dead, g.err, 5);
-      w = sh->sched_w[slot];  // plain load from a warp-uniform address (the wait above is a compiler barrier)
+      const int4 r = ptx::lds_s32x4(rec_a + 16 * slot);  // warp-uniform address
+      t.e = r.x; t.row0 = r.y; t.nrows = r.z; t.nt = r.w;
       if (whole_warp) {
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive_a(bar_a + kOffSchedEmpty + 8 * slot);
@@ -212,7 +230,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
         ptx::mbar_arrive_a(bar_a + kOffSchedEmpty + 8 * slot);
       }
     }
-    return w < total ? w : -1;
+    return t;
   };
 
   // Registers: 168 per thread at launch (384 threads); the producer / MMA warpgroup gives most of
@@ -224,13 +242,12 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
     if (ptx::elect_one()) {
       int stage = 0;
       uint32_t phase = 0;
-      Tile nx{0, 0, 0, 0};
+      Tile nx{-1, 0, 0, 0};
       if (w_first < total) nx = fetch(w_first);  // idle CTAs (and launches without any tile) read no record
-      int w = w_first < total ? w_first : -1;
-      for (int i = 0; w >= 0; ++i) {
+      int w = w_first;
+      for (int i = 0; nx.e >= 0; ++i) {
         const Tile cur = nx;
-        w = next_item(w, i, false);
-        if (w >= 0) nx = fetch(w);  // next tile's record is in flight during this tile's loads
+        nx = next_tile(w, i, false);
         const int e = cur.e, nt = cur.nt, row0 = cur.row0;
         const int slot = slot_of(g, e);
         constexpr int kBoxes = kPair ? 2 : 4;
@@ -238,11 +255,11 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
         if (kMode == 0) {
           // pool = [gate of all slots | up of all slots | down of all slots], viewed as [3 * slots * I, H]
           const int gate0 = slot * g.I + nt * 128, up0 = (g.n_slots + slot) * g.I + nt * 128;
-          if (kPair) { brow[0] = gate0 + 64 * rank; brow[1] = up0 + 64 * rank; }
+          if (kPair) { brow[0] = rank == 0 ? gate0 : up0; brow[1] = brow[0] + 64; }  // CTA 0: gate rows, CTA 1: up rows (64 per column half)
           else { brow[0] = gate0; brow[1] = up0; brow[2 % kBoxes] = gate0 + 64; brow[3 % kBoxes] = up0 + 64; }
         } else {
           const int down0 = (2 * g.n_slots + slot) * g.H + nt * BN;  // same pool viewed as [3 * slots * H, I]
-          if (kPair) { brow[0] = down0 + 128 * rank; brow[1] = brow[0] + 64; }
+          if (kPair) { brow[0] = down0 + 64 * rank; brow[1] = brow[0] + 128; }  // 64 rows of each column half
           else { brow[0] = down0; brow[1] = down0 + 64; brow[2 % kBoxes] = down0 + 128; brow[3 % kBoxes] = down0 + 192; }
         }
         for (int kb = 0; kb < num_kb; ++kb) {
@@ -272,7 +289,12 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
         const uint32_t slot = static_cast<uint32_t>(i) % kSchedDepth;
         ptx::mbar_wait_a(bar_a + kOffSchedEmpty + 8 * slot, ((static_cast<uint32_t>(i) / kSchedDepth) & 1) ^ 1, dead, g.err, 6);
         const int w = static_cast<int>(gridDim.x) + atomicAdd(g.sched + kMode, 1);
-        sh->sched_w[slot] = w;
+        int4 r = make_int4(-1, 0, 0, 0);
+        if (w < total) {
+          const Tile t = fetch(w);
+          r = make_int4(t.e, t.row0, t.nrows, t.nt);
+        }
+        ptx::sts_s32x4(rec_a + 16 * slot, r);
         ptx::mbar_arrive_a(bar_a + kOffSchedFull + 8 * slot);  // release: the store above is visible to the waiters
         if (w >= total) break;
       }
@@ -280,32 +302,39 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
    } else if (warp == kEpiWarps + 1) {
     // ===================== MMA issuer (one elected thread; pair: leader CTA only) =====================
     if (rank == 0 && ptx::elect_one()) {
-      constexpr uint32_t idesc = ptx::umma_idesc_e4m3_f32(kPair ? 2 * BM : BM, BN);
+      // A K block is issued as two N = 128 MMAs groups (columns [0, 128) and [128, 256) of the tile) with their own
+      // TMEM hand-off barriers: four 128-column buffers are in flight instead of two 256-column ones, so a half
+      // buffer has three MMA groups (768 cycles) to be drained and handed back before the tensor core needs it again,
+      // and the two promotion warps that share a scheduler work 256 cycles apart instead of in lock step.  Price: the
+      // A tile is read from shared memory twice per K block.
+      constexpr uint32_t idesc = ptx::umma_idesc_e4m3_f32(kPair ? 2 * BM : BM, HN);
+      constexpr uint64_t kHalfB = (kPair ? HN / 2 : HN) * BK / 16;  // B rows of column half 1 start here (16-byte units)
       const uint64_t adesc0 = ptx::umma_desc_k128_a(smem_a), bdesc0 = ptx::umma_desc_k128_a(smem_a + kABytes);
       int stage = 0;
       uint32_t phase = 0;
       uint32_t it = 0;  // running K-block counter: TMEM buffer = it & 1
-      int w = w_first < total ? w_first : -1;
-      for (int i = 0; w >= 0; w = next_item(w, i, false), ++i) {
+      int w = w_first;
+      bool have = w_first < total;
+      for (int i = 0; have; have = next_tile(w, i, false).e >= 0, ++i) {
         for (int kb = 0; kb < num_kb; ++kb, ++it) {
           const uint32_t buf = it & 1, tph = ((it >> 1) & 1) ^ 1;
           ptx::mbar_wait_a(bar_a + kOffFull + 8 * stage, phase, dead, g.err, 3);    // operands landed (usually long ago)
-          ptx::mbar_wait_a(bar_a + kOffTmemEmpty + 8 * buf, tph, dead, g.err, 2);   // the critical hand-off: issue right after it
-          ptx::tc_fence_after();
           const uint64_t so = static_cast<uint64_t>((stage * kStageBytes) >> 4);
-          const uint32_t d = tmem_base + buf * BN;
 #pragma unroll
-          for (int k4 = 0; k4 < BK / 32; ++k4) {  // UMMA_K = 32 for 8-bit operands: +32 B per step
-            if (kPair) ptx::umma_f8_2sm(d, adesc0 + so + 2 * k4, bdesc0 + so + 2 * k4, idesc, k4 > 0);
-            else ptx::umma_f8(d, adesc0 + so + 2 * k4, bdesc0 + so + 2 * k4, idesc, k4 > 0);
+          for (int h = 0; h < 2; ++h) {
+            ptx::mbar_wait_a(bar_a + kOffTmemEmpty + 16 * buf + 8 * h, tph, dead, g.err, 2);   // the hand-off: issue right after it
+            ptx::tc_fence_after();
+            const uint32_t d = tmem_base + buf * BN + h * HN;
+#pragma unroll
+            for (int k4 = 0; k4 < BK / 32; ++k4) {  // UMMA_K = 32 for 8-bit operands: +32 B per step
+              if (kPair) ptx::umma_f8_2sm(d, adesc0 + so + 2 * k4, bdesc0 + so + h * kHalfB + 2 * k4, idesc, k4 > 0);
+              else ptx::umma_f8(d, adesc0 + so + 2 * k4, bdesc0 + so + h * kHalfB + 2 * k4, idesc, k4 > 0);
+            }
+            if (kPair) ptx::umma_commit_2sm_mc(bar_a + kOffTmemFull + 16 * buf + 8 * h, 3);  // both CTAs' rows of this half are complete
+            else ptx::umma_commit_a(bar_a + kOffTmemFull + 16 * buf + 8 * h);
           }
-          if (kPair) {
-            ptx::umma_commit_2sm_mc(bar_a + kOffTmemFull + 8 * buf, 3);  // both CTAs' halves of the partial are complete
-            ptx::umma_commit_2sm_mc(bar_a + kOffEmpty + 8 * stage, 3);   // both CTAs' stages reusable once these MMAs retire
-          } else {
-            ptx::umma_commit_a(bar_a + kOffTmemFull + 8 * buf);
-            ptx::umma_commit_a(bar_a + kOffEmpty + 8 * stage);
-          }
+          if (kPair) ptx::umma_commit_2sm_mc(bar_a + kOffEmpty + 8 * stage, 3);   // both CTAs' stages reusable once these MMAs retire
+          else ptx::umma_commit_a(bar_a + kOffEmpty + 8 * stage);
           if (++stage == kStages) { stage = 0; phase ^= 1; }
         }
       }
@@ -319,12 +348,17 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
     const uint32_t tm_lane = ptx::launder_u32(tmem_base + (static_cast<uint32_t>(q * 32) << 16) + half * HN);
     uint32_t it = 0;
     int tile_parity = 0;
-    const uint32_t te_a = lead_bar + kOffTmemEmpty;  // pair: the leader's barrier (cluster address)
-    // Per-tile scale pointers; the first loads of a tile are issued before the previous tile's epilogue.
+    const uint32_t te_a = lead_bar + kOffTmemEmpty + 8 * half;  // [buffer][this warp's column half]; pair: the leader's barrier (cluster address)
+    const uint32_t tf_a = bar_a + kOffTmemFull + 8 * half;
+    // Per-tile scales.  The row's activation scales xs[row, kb] come as one 16-byte load per four K blocks (issued
+    // four K blocks ahead); the weight scales (ws0[kb], ws1[kb]) of the tile go through a small per-warp table in
+    // shared memory: lane l fetches K blocks l and l + 32 while the previous tile's epilogue runs, the table is
+    // written at the start of the K loop and every K block costs one 8-byte shared load at a warp-uniform address.
     const float *as_ptr = nullptr, *ws0 = nullptr, *ws1 = nullptr;
     bool row_ok = false;
     float4 xs_nxt = make_float4(0.f, 0.f, 0.f, 0.f);
-    float w0_nxt = 0.f, w1_nxt = 0.f;
+    float wa0 = 0.f, wa1 = 0.f, wb0 = 0.f, wb1 = 0.f;  // prefetched weight scales: K blocks lane (a) and lane + 32 (b)
+    const uint32_t wsm_a = ptx::launder_u32(smem_a + kStages * kStageBytes + C::kYBytes + warp * (kWsCap * 8));  // this warp's table
     auto open_tile = [&](const Tile& t) {
       row_ok = r_in_tile < t.nrows;
       as_ptr = g.a_s + static_cast<size_t>(t.row0 + r_in_tile) * g.a_s_stride;  // padded to a multiple of 4 floats, 16-byte aligned
@@ -338,125 +372,116 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
         ws0 = g.down_s + (static_cast<size_t>(t.e) * (g.H / 128) + nb) * num_kb;
         ws1 = ws0;
       }
-      // Scales are fetched far ahead of use: the row's activation scales four K blocks at a time
-      // (one 16-byte load), the weight scales 32 K blocks at a time, one per lane, broadcast by shuffle.
       xs_nxt = row_ok ? *reinterpret_cast<const float4*>(as_ptr) : make_float4(0.f, 0.f, 0.f, 0.f);
-      w0_nxt = lane < num_kb ? ws0[lane] : 0.f;
-      w1_nxt = (kMode == 0 && lane < num_kb) ? ws1[lane] : 0.f;
+      wa0 = lane < num_kb ? ws0[lane] : 0.f;
+      wb0 = lane + 32 < num_kb ? ws0[lane + 32] : 0.f;
+      if (kMode == 0) {
+        wa1 = lane < num_kb ? ws1[lane] : 0.f;
+        wb1 = lane + 32 < num_kb ? ws1[lane + 32] : 0.f;
+      }
     };
-    Tile nx{0, 0, 0, 0};
+    // weight scales of K blocks [k0, k0 + kWsCap) of the open tile -> table (k0 > 0 only when num_kb > kWsCap)
+    auto refill_ws = [&](int k0) {
+      __syncwarp();
+      for (int k = lane; k < kWsCap; k += 32) {
+        const int kk = k0 + k;
+        ptx::sts_f32x2(wsm_a + 8 * k, kk < num_kb ? ws0[kk] : 0.f, (kMode == 0 && kk < num_kb) ? ws1[kk] : 0.f);
+      }
+      __syncwarp();
+    };
+    Tile nx{-1, 0, 0, 0};
     if (w_first < total) { nx = fetch(w_first); open_tile(nx); }
-    int w = w_first < total ? w_first : -1;
+    int w = w_first;
 #ifdef SLP_PROF
     long long pk = 0, pe = 0, pf = 0, pn = 0, pq = 0;
 #endif
-    for (int i = 0; w >= 0; ++i, tile_parity ^= 1) {
-#ifdef SLP_PROF
-      const long long p0 = clock64();
-      long long p1 = p0;
-#endif
+    for (int ti = 0; nx.e >= 0; ++ti, tile_parity ^= 1) {
       const Tile cur = nx;
-      w = next_item(w, i, true);
-      const bool has_next = w >= 0;
-      if (has_next) nx = fetch(w);  // record in flight during the K loop
 #ifdef SLP_PROF
       const long long pa = clock64();
+      long long p1 = pa;
 #endif
       const int nt = cur.nt, row0 = cur.row0, nrows = cur.nrows;
       const size_t row = static_cast<size_t>(row0 + r_in_tile);
       const bool row_ok_cur = row_ok;
-      uint64_t acc2[64];  // 128 fp32 accumulators as FFMA2 pairs
+      float acc[128];  // fp32 accumulators, updated in FFMA2 pairs
 #pragma unroll
-      for (int i = 0; i < 64; ++i) acc2[i] = 0ull;
+      for (int i = 0; i < 128; ++i) acc[i] = 0.f;
+      __syncwarp();  // every lane is done reading the previous tile's table
+      ptx::sts_f32x2(wsm_a + 8 * lane, wa0, wa1);
+      ptx::sts_f32x2(wsm_a + 8 * (lane + 32), wb0, wb1);
+      __syncwarp();
 
-      float w0_cur = 0.f, w1_cur = 0.f;
-      float4 xs_cur = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll 1
-      for (int kb = 0; kb < num_kb; ++kb) {
-        {
-          // Branch-free scale bookkeeping (selp): a branchy version cost ~40 MOV / BRA per K block in
-          // an issue-bound loop.  Every 4th K block the row's next four activation scales (one 16-byte
-          // load issued a group ahead) become current; every 32nd the lane-held weight scales rotate.
-          const int j = kb & 3;
-          const bool g4 = j == 0, g32 = (kb & 31) == 0;
-          xs_cur.x = sel_f32(g4, xs_nxt.x, xs_cur.x);
-          xs_cur.y = sel_f32(g4, xs_nxt.y, xs_cur.y);
-          xs_cur.z = sel_f32(g4, xs_nxt.z, xs_cur.z);
-          xs_cur.w = sel_f32(g4, xs_nxt.w, xs_cur.w);
-          w0_cur = sel_f32(g32, w0_nxt, w0_cur);
-          w1_cur = sel_f32(g32, w1_nxt, w1_cur);
-          if (g4) {
-            if (kb + 4 < num_kb && row_ok) xs_nxt = *reinterpret_cast<const float4*>(as_ptr + kb + 4);
-            if (g32) {
-              const int kn = kb + 32 + lane;
-              w0_nxt = kn < num_kb ? ws0[kn] : 0.f;
-              w1_nxt = (kMode == 0 && kn < num_kb) ? ws1[kn] : 0.f;
-            }
-          }
-          const float sa = sel_f32((j & 2) != 0, sel_f32((j & 1) != 0, xs_cur.w, xs_cur.z), sel_f32((j & 1) != 0, xs_cur.y, xs_cur.x));
-          const float sc0 = sa * __shfl_sync(0xFFFFFFFFu, w0_cur, kb & 31);
-          const float sc1 = kMode == 0 ? sa * __shfl_sync(0xFFFFFFFFu, w1_cur, kb & 31) : sc0;
-          const uint64_t s20 = ptx::pack2(sc0, sc0), s21 = ptx::pack2(sc1, sc1);
-          const uint32_t buf = it & 1;
-          ptx::mbar_wait_a(bar_a + kOffTmemFull + 8 * buf, (it >> 1) & 1, dead, g.err, 4);
-          ptx::tc_fence_after();
+      // One K block: the warp waits for the partial of ITS column half in TMEM buffer it & 1 (the MMA issuer
+      // publishes the two 128-column halves of a K block separately, see there), pulls the thread's 128 columns out
+      // in 8 chunks of 16 through four register sets and adds them, scaled, into the accumulators.  Chunks 0-3 are
+      // requested up front, chunk c + 4 as soon as the FMAs of chunk c have consumed its set, so every tcgen05.ld of
+      // the K block has landed after half of the FMAs and the half-buffer goes back to the MMA issuer there.
+      auto k_block = [&](float sa, int kb) {
+        const float2 wsc = ptx::lds_f32x2(wsm_a + 8 * (kb & (kWsCap - 1)));  // warp-uniform address; lands during the wait below
+        const uint32_t buf = it & 1;
+        ptx::mbar_wait_a(tf_a + 16 * buf, (it >> 1) & 1, dead, g.err, 4);
+        ptx::tc_fence_after();
 #ifdef SLP_PROF
-          if (kb == 0) p1 = clock64();
+        if (kb == 0) p1 = clock64();
 #endif
-          const uint32_t tb = tm_lane + buf * BN;
-          {
-            // 8 chunks of 16 columns through four register sets: chunks 0-3 are loaded up front, chunk
-            // c + 4 is requested as soon as the FMAs of chunk c have consumed its set, so every
-            // tcgen05.ld of the K block has landed after half of the FMAs and the TMEM buffer goes back
-            // to the MMA issuer there.  The K loop is bound by the hand-off round trip, not by throughput:
-            // time per K block = (MMA 512 + ~500 cycles of commit / wake-up / issue latency + drain) / 2
-            // with two TMEM buffers, drain = buffer published -> buffer released.
-            uint32_t v[4][16];
-  #pragma unroll
-            for (int c = 0; c < 4; ++c) ptx::tmem_ld16(tb + c * 16, v[c]);
-            ptx::tmem_ld_wait16(v[0]);
-            ptx::keep16(v[1]); ptx::keep16(v[2]); ptx::keep16(v[3]);
-  #pragma unroll
-            for (int c = 0; c < 4; ++c) {
-              const uint64_t s2 = s20;  // chunks 0-3: gate columns (mode 0) / first weight-scale block
-  #pragma unroll
-              for (int i = 0; i < 16; i += 2) ptx::fma2(acc2[c * 8 + i / 2], v[c][i], v[c][i + 1], s2);
-              ptx::tmem_ld16(tb + (c + 4) * 16, v[c]);
-            }
-            ptx::tmem_ld_wait16(v[0]);
-            ptx::keep16(v[1]); ptx::keep16(v[2]); ptx::keep16(v[3]);
-            // the whole partial is in registers: hand the TMEM buffer back before the last FMAs
-            ptx::tc_fence_before();
-            __syncwarp();
-            if (lane == 0) {
-              if (kPair && rank != 0) ptx::mbar_arrive_cluster(te_a + 8 * buf);  // remote: the leader's barrier
-              else ptx::mbar_arrive_a(bar_a + kOffTmemEmpty + 8 * buf);
-            }
-  #pragma unroll
-            for (int c = 0; c < 4; ++c) {
-              const uint64_t s2 = s21;  // chunks 4-7: up columns (mode 0) / same block (mode 1: s21 == s20)
-  #pragma unroll
-              for (int i = 0; i < 16; i += 2) ptx::fma2(acc2[(c + 4) * 8 + i / 2], v[c][i], v[c][i + 1], s2);
-            }
-          }
-          ++it;
+        const uint32_t tb = tm_lane + buf * BN;
+        uint32_t v[4][16];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) ptx::tmem_ld16(tb + c * 16, v[c]);
+        const float sc0 = sa * wsc.x;                           // gate columns (mode 0) / the one weight-scale block (mode 1)
+        const float sc1 = kMode == 0 ? sa * wsc.y : sc0;        // up columns (mode 0)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+#pragma unroll
+          for (int i = 0; i < 16; i += 2) ptx::fma2f(acc[c * 16 + i], acc[c * 16 + i + 1], v[c][i], v[c][i + 1], sc0);
+          ptx::tmem_ld16(tb + (c + 4) * 16, v[c]);
         }
+        ptx::tmem_ld_wait();
+        // the whole partial is in registers: hand the TMEM half-buffer back before the last FMAs
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) {
+          if (kPair && rank != 0) ptx::mbar_arrive_cluster(te_a + 16 * buf);  // remote: the leader's barrier
+          else ptx::mbar_arrive_a(te_a + 16 * buf);
+        }
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+#pragma unroll
+          for (int i = 0; i < 16; i += 2) ptx::fma2f(acc[(c + 4) * 16 + i], acc[(c + 4) * 16 + i + 1], v[c][i], v[c][i + 1], sc1);
+        }
+        ++it;
+      };
+
+#pragma unroll 1
+      for (int kb0 = 0; kb0 < num_kb; kb0 += 4) {
+        if (kb0 != 0 && (kb0 & (kWsCap - 1)) == 0) refill_ws(kb0);
+        const float4 xs4 = xs_nxt;
+        if (kb0 + 4 < num_kb && row_ok) xs_nxt = *reinterpret_cast<const float4*>(as_ptr + kb0 + 4);
+        k_block(xs4.x, kb0);
+        if (kb0 + 1 < num_kb) k_block(xs4.y, kb0 + 1);
+        if (kb0 + 2 < num_kb) k_block(xs4.z, kb0 + 2);
+        if (kb0 + 3 < num_kb) k_block(xs4.w, kb0 + 3);
       }
 #ifdef SLP_PROF
       const long long p2 = clock64();
 #endif
-      if (has_next) open_tile(nx);  // first scale loads of the next tile fly during this tile's epilogue
-      float acc[128];
-#pragma unroll
-      for (int i = 0; i < 64; ++i) ptx::unpack2(acc2[i], acc[2 * i], acc[2 * i + 1]);
+#ifdef SLP_PROF
+      const long long q0 = clock64();
+#endif
+      nx = next_tile(w, ti, true);   // one barrier wait + one 16-byte shared load (the scheduler warp read the record)
+      if (nx.e >= 0) open_tile(nx);  // first scale loads of the next tile fly during this tile's epilogue
+#ifdef SLP_PROF
+      pq += clock64() - q0;
+#endif
 
       if (kMode == 0) {
         // h = silu(gate) * up over this thread's 64 channels; row amax over all 128 via smem
         float amax = 0.f;
 #pragma unroll
-        for (int i = 0; i < 64; ++i) {
-          acc[i] = silu_mul_fast(acc[i], acc[64 + i]);
-          amax = fmaxf(amax, fabsf(acc[i]));
+        for (int i = 0; i < 64; i += 2) {
+          silu_mul_fast2(acc[i], acc[64 + i], acc[i + 1], acc[64 + i + 1]);
+          amax = fmaxf(amax, fmaxf(fabsf(acc[i]), fabsf(acc[i + 1])));
         }
         float* ex = reinterpret_cast<float*>(scratch) + tile_parity * 2 * BM;  // [parity][half][row]
         ex[half * BM + r_in_tile] = amax;
@@ -530,7 +555,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
         }
       }
 #ifdef SLP_PROF
-      { const long long p3 = clock64(); pf += p1 - pa; pq += pa - p0; pk += p2 - p1; pe += p3 - p2; pn += 1; }
+      { const long long p3 = clock64(); pf += p1 - pa; pk += p2 - p1; pe += p3 - p2; pn += 1; }
 #endif
     }
 #ifdef SLP_PROF

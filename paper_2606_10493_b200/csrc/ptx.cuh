@@ -185,6 +185,12 @@ __device__ __forceinline__ void keep16(uint32_t (&v)[16]) {
                  "+r"(v[8]), "+r"(v[9]), "+r"(v[10]), "+r"(v[11]), "+r"(v[12]), "+r"(v[13]), "+r"(v[14]), "+r"(v[15]));
 }
 
+// Empty statement that only READS 16 registers: keeps them live up to this point.
+__device__ __forceinline__ void use16(const uint32_t (&v)[16]) {
+  asm volatile("" :: "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]),
+                     "r"(v[8]), "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]));
+}
+
 // ---- shared-address variants -------------------------------------------------------------------
 // The hot loops keep every barrier / stage address as a 32-bit shared-window address computed once
 // (a generic pointer would be re-converted with S2UR/ULEA sequences at every use).
@@ -200,6 +206,16 @@ __device__ __forceinline__ bool mbar_try_wait_a(uint32_t bar, uint32_t parity) {
   asm volatile(
       "{\n\t.reg .pred p;\n\t"
       "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+  return ok != 0;
+}
+// Non-blocking probe of a phase (test_wait never suspends the thread).
+__device__ __forceinline__ bool mbar_test_wait_a(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
       "selp.u32 %0, 1, 0, p;\n\t}"
       : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
   return ok != 0;
@@ -247,6 +263,25 @@ __device__ __forceinline__ uint64_t umma_desc_k128_a(uint32_t smem_addr) {
   return d;
 }
 
+// 8-byte shared-memory accesses through a 32-bit shared-window address
+__device__ __forceinline__ float2 lds_f32x2(uint32_t addr) {
+  float2 r;
+  asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(r.x), "=f"(r.y) : "r"(addr) : "memory");
+  return r;
+}
+__device__ __forceinline__ void sts_f32x2(uint32_t addr, float x, float y) {
+  asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(addr), "f"(x), "f"(y) : "memory");
+}
+
+__device__ __forceinline__ int4 lds_s32x4(uint32_t addr) {
+  int4 r;
+  asm volatile("ld.shared.v4.s32 {%0, %1, %2, %3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(addr) : "memory");
+  return r;
+}
+__device__ __forceinline__ void sts_s32x4(uint32_t addr, int4 v) {
+  asm volatile("st.shared.v4.s32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
 // Two fp32 FMAs in one instruction (FFMA2): (a0, a1) += (v0, v1) * (s, s).  `s2` holds the scale in
 // both halves.  Halves the issue slots of the block-scale promotion; ptxas allocates the pairs in
 // place (tcgen05.ld destinations and accumulators are consecutive even-aligned registers).
@@ -260,6 +295,20 @@ __device__ __forceinline__ void fma2(uint64_t& acc, uint32_t v0, uint32_t v1, ui
       "{\n\t.reg .b64 a;\n\tmov.b64 a, {%1, %2};\n\t"
       "fma.rn.f32x2 %0, a, %3, %0;\n\t}"
       : "+l"(acc) : "r"(v0), "r"(v1), "l"(s2));
+}
+// Same with a scalar scale: ptxas emits the broadcast form (FFMA2 ... Rs.F32 ...), no packed copy of the scale.
+__device__ __forceinline__ void fma2s(uint64_t& acc, uint32_t v0, uint32_t v1, float s) {
+  asm volatile(
+      "{\n\t.reg .b64 a, b;\n\tmov.b64 a, {%1, %2};\n\tmov.b64 b, {%3, %3};\n\t"
+      "fma.rn.f32x2 %0, a, b, %0;\n\t}"
+      : "+l"(acc) : "r"(v0), "r"(v1), "f"(s));
+}
+// Same on two separate fp32 accumulators (the pair is formed inside the statement).
+__device__ __forceinline__ void fma2f(float& a0, float& a1, uint32_t v0, uint32_t v1, float s) {
+  asm volatile(
+      "{\n\t.reg .b64 a, b, c;\n\tmov.b64 a, {%2, %3};\n\tmov.b64 b, {%4, %4};\n\tmov.b64 c, {%0, %1};\n\t"
+      "fma.rn.f32x2 c, a, b, c;\n\tmov.b64 {%0, %1}, c;\n\t}"
+      : "+f"(a0), "+f"(a1) : "r"(v0), "r"(v1), "f"(s));
 }
 // (lo, hi) fp32 -> packed f16x2, round to nearest even; lo lands in the low half (the lower address)
 __device__ __forceinline__ uint32_t pack_f16x2(float lo, float hi) {

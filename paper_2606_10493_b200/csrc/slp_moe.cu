@@ -821,6 +821,7 @@ extern "C" {
 const char* slp_last_error(void) { return g_last_error.c_str(); }
 const char* slp_version(void) { return "slpmoe 0.1 (sm_100a)"; }
 
+
 slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weights* w, slp_moe_layer** out) {
   return slp_moe_stack_create(cfg, 1, w, out);
 }
@@ -1343,7 +1344,7 @@ slp_status slp_moe_get_stats(slp_moe_layer* h, slp_moe_stats* stats) {
 #ifdef SLP_PROF
     for (int m = 0; m < 2; ++m)
       if (clk[7 + 4 * m])
-        fprintf(stderr, "[slp prof] mode %d: tiles/CTA-warp0 %llu, per tile: next-item %.0f, first-wait %.0f, K loop %.0f, epilogue %.0f cycles\n", m,
+        fprintf(stderr, "[slp prof] mode %d: tiles/CTA-warp0 %llu, per tile: next tile + scale prefetch %.0f, first-wait %.0f, K loop %.0f, epilogue %.0f cycles\n", m,
                 clk[7 + 4 * m], double(clk[12 + m]) / clk[7 + 4 * m], double(clk[4 + 4 * m]) / clk[7 + 4 * m], double(clk[5 + 4 * m]) / clk[7 + 4 * m], double(clk[6 + 4 * m]) / clk[7 + 4 * m]);
 #endif
     h->stats.sm_mhz_gateup = clk[1] ? static_cast<float>(1e3 * static_cast<double>(clk[0]) / static_cast<double>(clk[1])) : 0.f;
