@@ -318,11 +318,19 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
       for (int i = 0; have; have = next_tile(w, i, false).e >= 0, ++i) {
         for (int kb = 0; kb < num_kb; ++kb, ++it) {
           const uint32_t buf = it & 1, tph = ((it >> 1) & 1) ^ 1;
-          ptx::mbar_wait_a(bar_a + kOffFull + 8 * stage, phase, dead, g.err, 3);    // operands landed (usually long ago)
+          // A barrier probe takes ~100 cycles to answer even when the phase completed long ago, and this one thread
+          // needs three answers per K block: the three probes are issued back to back (test_wait never suspends the
+          // thread) and only a phase that is still open is then waited for.  Waiting for them one after the other made
+          // this loop, not the tensor core, the bound of the kernel (~500 cycles per K block).
+          const uint32_t fa = bar_a + kOffFull + 8 * stage, e0a = bar_a + kOffTmemEmpty + 16 * buf, e1a = e0a + 8;
+          const bool pf = ptx::mbar_test_wait_a(fa, phase);
+          const bool p0 = ptx::mbar_test_wait_a(e0a, tph);
+          const bool p1 = ptx::mbar_test_wait_a(e1a, tph);
+          if (!pf) ptx::mbar_wait_a(fa, phase, dead, g.err, 3);   // operands landed (usually long ago)
           const uint64_t so = static_cast<uint64_t>((stage * kStageBytes) >> 4);
 #pragma unroll
           for (int h = 0; h < 2; ++h) {
-            ptx::mbar_wait_a(bar_a + kOffTmemEmpty + 16 * buf + 8 * h, tph, dead, g.err, 2);   // the hand-off: issue right after it
+            if (!(h == 0 ? p0 : p1)) ptx::mbar_wait_a(h == 0 ? e0a : e1a, tph, dead, g.err, 2);   // the hand-off: issue right after it
             ptx::tc_fence_after();
             const uint32_t d = tmem_base + buf * BN + h * HN;
 #pragma unroll
