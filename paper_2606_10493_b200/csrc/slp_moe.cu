@@ -105,6 +105,8 @@ inline int auto_epl(int n_stage, int E) {
   return best;
 }
 
+constexpr int kTailExperts = 8;  // experts per launch inside the last launch group of a streamed call (prefill_impl)
+
 inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
 
 // Triage switches, read once per create from the environment variable SLP_TRIAGE (comma-separated tokens);
@@ -236,6 +238,7 @@ struct slp_moe_layer {
   slp_moe_stats stats{};
   bool stats_copy_valid = false;
   std::vector<cudaEvent_t> ev_k;  // 3 events per expert launch pair: before gate/up, between, after down
+  std::vector<cudaEvent_t> ev_tail;  // ON events of the pieces of a call's last launch group
   int ev_k_used = 0;
 };
 
@@ -739,6 +742,38 @@ slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t
         }
         for (int e = e0; e < e1; ++e)
           if (skip && h->h_counts[e] == 0) h->stats.experts_skipped += 1;
+        // The call ends one group's compute after the last copy has landed.  The LAST group of a call is therefore
+        // copied and launched in pieces of kTailExperts experts, each launch waiting only for its own piece: the tail
+        // shrinks from the compute of a whole group (3.3 ms of a 32K-token call with 64 experts per launch) to that
+        // of a piece, while every other group keeps the large launches that amortise the launch ramp.
+        const bool last_group = e1 == e_own1 && e1 - e0 > kTailExperts && !h->ev_tail.empty();
+        if (last_group) {
+          int piece = 0;
+          for (int p0 = e0; p0 < e1; p0 += kTailExperts, ++piece) {
+            const int p1 = std::min(e1, p0 + kTailExperts);
+            int pneed = 0, prows = 0;
+            for (int e = p0; e < p1; ++e) {
+              pneed += (!skip || h->h_counts[e] > 0) ? 1 : 0;
+              if (skip) prows += (h->h_counts[e] + 127) / 128;
+            }
+            if (pneed == 0) continue;
+            slp_status st = copy_experts(h, p0, p1, skip ? h->h_counts : nullptr);
+            if (st != SLP_OK) return st;
+            cudaEvent_t ev = h->ev_tail[piece % h->ev_tail.size()];
+            CU_TRY(cudaEventRecord(ev, h->copy_stream));
+            CU_TRY(cudaStreamWaitEvent(s, ev, 0));
+            const int pbound = skip ? prows : std::min(routed_tiles_bound, (T * k) / 128 + (p1 - p0));
+            st = launch_experts(h, s, p0, p1, T, std::max(1, pbound));
+            if (st != SLP_OK) return st;
+          }
+          h->occ_layer[r] = layer;
+          h->occ_e0[r] = e0;
+          h->occ_prefetched[r] = 0;
+          CU_TRY(cudaEventRecord(h->ev_ready[r], h->copy_stream));  // ON for the whole group (bookkeeping of later calls)
+          CU_TRY(cudaEventRecord(h->ev_free[r], s));  // OFF
+          h->free_recorded[r] = 1;
+          continue;
+        }
         {
           slp_status st = copy_experts(h, e0, e1, skip ? h->h_counts : nullptr);
           if (st != SLP_OK) return st;
@@ -903,6 +938,8 @@ slp_status slp_moe_stack_create(const slp_moe_cfg* cfg, int32_t n_layers, const 
   CU_OR_BAIL(cudaEventCreate(&h->ev_copy1));
   h->ev_k.resize(3 * (E + 2));
   for (auto& e : h->ev_k) CU_OR_BAIL(cudaEventCreate(&e));
+  h->ev_tail.resize(64);
+  for (auto& e : h->ev_tail) CU_OR_BAIL(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
 
   // ---- per layer: pin (or check) the streamed weights, upload router / bias / block scales / shared expert ----
   CU_OR_BAIL(cudaFuncSetAttribute(slp::rtc::router_logits_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::rtc::kSmemBytes));
@@ -1044,7 +1081,11 @@ slp_status slp_moe_query_plan(const slp_moe_cfg* cfg, slp_moe_plan* plan) {
   plan->staging_slots = n_stage;
   plan->experts_per_launch = epl;
   const int64_t En = cfg->expert_end == 0 ? E : cfg->expert_end - cfg->expert_begin;
-  plan->launch_pairs_streamed = static_cast<int32_t>((En + epl - 1) / epl + (cfg->n_shared ? 1 : 0));
+  {  // the last group is launched in pieces of kTailExperts experts (prefill_impl)
+    const int groups = (En + epl - 1) / epl, last = En - (groups - 1) * epl;
+    const int last_launches = last > kTailExperts ? (last + kTailExperts - 1) / kTailExperts : 1;
+    plan->launch_pairs_streamed = static_cast<int32_t>(groups - 1 + last_launches + (cfg->n_shared ? 1 : 0));
+  }
   plan->workspace_rows = rows;
   plan->expert_slot_bytes = 3 * I * H;
   plan->routed_bytes_per_pass = En * 3 * I * H;
@@ -1233,6 +1274,8 @@ slp_status slp_moe_layer_destroy(slp_moe_layer* h) {
   if (h->ev_copy0) cudaEventDestroy(h->ev_copy0);
   if (h->ev_copy1) cudaEventDestroy(h->ev_copy1);
   for (auto e : h->ev_k)
+    if (e) cudaEventDestroy(e);
+  for (auto e : h->ev_tail)
     if (e) cudaEventDestroy(e);
   cudaGetLastError();
   delete h;
