@@ -139,8 +139,9 @@ typedef struct {
   uint32_t struct_size;            /* = sizeof(slp_moe_plan) */
   int32_t staging_slots;           /* expert slots of the streamed ring after defaults (0 -> n_experts) */
   int32_t experts_per_launch;      /* experts per grouped-GEMM launch pair after defaults */
-  int32_t launch_pairs_streamed;   /* gate/up + down launch pairs per streamed call (incl. the shared expert; the last
-                                      group of a call is launched in pieces of 8 experts to shorten the call's tail) */
+  int32_t launch_pairs_streamed;   /* gate/up + down launch pairs of a streamed call of max_tokens tokens (incl. the shared
+                                      expert; with >= 256 rows per expert the last group of a call is launched in pieces
+                                      of 8 experts to shorten the call's tail) */
   int64_t workspace_rows;          /* rows of xq / hq / Y: padded tokens + 128-aligned expert ranges */
   int64_t expert_slot_bytes;       /* 3 * I * H: gate | up | down of one expert ("3 FP8 linears") */
   int64_t routed_bytes_per_pass;   /* E * 3 * I * H: what one streamed call moves over the host link */

@@ -742,11 +742,14 @@ slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t
         }
         for (int e = e0; e < e1; ++e)
           if (skip && h->h_counts[e] == 0) h->stats.experts_skipped += 1;
-        // The call ends one group's compute after the last copy has landed.  The LAST group of a call is therefore
+        // The call ends one group's compute after the last copy has landed.  The LAST group of a long call is therefore
         // copied and launched in pieces of kTailExperts experts, each launch waiting only for its own piece: the tail
         // shrinks from the compute of a whole group (3.3 ms of a 32K-token call with 64 experts per launch) to that
         // of a piece, while every other group keeps the large launches that amortise the launch ramp.
-        const bool last_group = e1 == e_own1 && e1 - e0 > kTailExperts && !h->ev_tail.empty();
+        // Only where it pays: with fewer than ~256 rows per expert the GEMMs are HBM-bound, the whole group's compute is
+        // well under a millisecond and small launches would only add launch ramps.
+        const bool last_group = e1 == e_own1 && e1 - e0 > kTailExperts && !h->ev_tail.empty() &&
+                                static_cast<long long>(T) * k >= 256LL * E;
         if (last_group) {
           int piece = 0;
           for (int p0 = e0; p0 < e1; p0 += kTailExperts, ++piece) {
@@ -1081,9 +1084,10 @@ slp_status slp_moe_query_plan(const slp_moe_cfg* cfg, slp_moe_plan* plan) {
   plan->staging_slots = n_stage;
   plan->experts_per_launch = epl;
   const int64_t En = cfg->expert_end == 0 ? E : cfg->expert_end - cfg->expert_begin;
-  {  // the last group is launched in pieces of kTailExperts experts (prefill_impl)
+  {  // the last group of a long call (>= 256 rows per expert) is launched in pieces of kTailExperts experts (prefill_impl)
     const int groups = (En + epl - 1) / epl, last = En - (groups - 1) * epl;
-    const int last_launches = last > kTailExperts ? (last + kTailExperts - 1) / kTailExperts : 1;
+    const bool pieces = last > kTailExperts && static_cast<long long>(cfg->max_tokens) * cfg->top_k >= 256LL * cfg->n_experts;
+    const int last_launches = pieces ? (last + kTailExperts - 1) / kTailExperts : 1;
     plan->launch_pairs_streamed = static_cast<int32_t>(groups - 1 + last_launches + (cfg->n_shared ? 1 : 0));
   }
   plan->workspace_rows = rows;

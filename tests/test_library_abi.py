@@ -84,7 +84,9 @@ def test_query_plan_byte_accounting_matches_the_paper(built):
     assert p["expert_slot_bytes"] == 3 * 2048 * 7168 == 44040192
     assert p["routed_bytes_per_pass"] == 11274289152 and round(p["routed_bytes_per_pass"] / 1e9, 1) == 11.3
     assert p["staging_slots"] == 256 and p["pool_bytes_streamed"] == 257 * 44040192 == p["pool_bytes_resident"]
-    assert p["experts_per_launch"] == 64 and p["launch_pairs_streamed"] == 3 + 8 + 1   # last group in 8-expert pieces
+    assert p["experts_per_launch"] == 64 and p["launch_pairs_streamed"] == 4 + 1        # T = 4096: 128 rows per expert, whole groups
+    p32 = binding.query_plan(inputs.CONFIGS[2])                                         # T = 32768: the last group goes in 8-expert pieces
+    assert p32["experts_per_launch"] == 64 and p32["launch_pairs_streamed"] == 3 + 8 + 1
     assert p["scale_bytes"] == 257 * 3 * 16 * 56 * 4
     assert p["fp8_flops_per_token"] == 2 * 3 * 2048 * 7168 * 9 == inputs.fp8_flops_per_token(inputs.CONFIGS[1])
     assert p["workspace_rows"] == 4096 + (4096 * 8 + 256 * 127 + 127) // 128 * 128
