@@ -10,8 +10,12 @@
 // accumulation is the tensor core's fp32; the logit error stays near 1e-5 (measured in the parity
 // tests through the SLP_BUF_LOGITS export), a decade below the near-tie allowance.
 //
-//   grid   (ceil(T / 128), ceil(E / 256)); one 128-token x <=256-expert tile per CTA
-//   warp 4 TMA producer: x tile (128 rows x 64 bf16) + hi and lo tiles of W_r per K step,
+//   grid   (ceil(T / (128 kRowTiles)), ceil(E / 256)); kRowTiles 128-token x <=256-expert tiles per CTA.  Every CTA
+//          streams the whole split W_r (7.3 MB for 256 x 7168) through its shared memory, so with one row tile per
+//          CTA the kernel is bound by L2 -> SM traffic (2.35 GB through the crossbar for 0.48 GB of DRAM at 32K
+//          tokens); two row tiles per CTA (two fp32 accumulators = all 512 TMEM columns) halve it.  The host picks
+//          kRowTiles = 2 when one row tile per CTA would need more than one wave of CTAs.
+//   warp 4 TMA producer: kRowTiles x tiles (128 rows x 64 bf16) + hi and lo tiles of W_r per K step,
 //          128B-swizzled 2-stage ring
 //   warp 5 MMA issuer: 4 K sub-steps x {hi, lo} tcgen05.mma.kind::f16 (M128, N = tile experts)
 //   warps 0-3 epilogue: tcgen05.ld -> fp32 logits rows
@@ -27,9 +31,12 @@ namespace rtc {
 constexpr int BM = 128, BKB = 128 /* bytes of K per step = 64 bf16 */, BN = 256;
 constexpr int kStages = 2;
 constexpr int kABytes = BM * BKB, kBoxBytes = 128 * BKB;
-constexpr int kStageBytes = kABytes + 4 * kBoxBytes;  // A | hi (2 boxes) | lo (2 boxes)
 constexpr int kThreads = 192;
-constexpr int kSmemBytes = kStages * kStageBytes + 1024 /*align*/ + 128 /*barriers*/;
+template <int kRowTiles> struct Cfg {
+  static constexpr int kStageBytes = kRowTiles * kABytes + 4 * kBoxBytes;  // A tiles | hi (2 boxes) | lo (2 boxes)
+  static constexpr int kSmemBytes = kStages * kStageBytes + 1024 /*align*/ + 128 /*barriers*/;
+  static_assert(kSmemBytes <= 232448, "shared memory budget");
+};
 
 // W_r [E, H] fp32 -> hl [2][Erows][H] bf16 bit patterns (hi, then lo = bf16(w - hi)); rows >= E stay 0.
 __global__ void __launch_bounds__(256) split_router_w_kernel(const float* __restrict__ w, uint16_t* __restrict__ hl, int E, int H,
@@ -54,14 +61,18 @@ struct Shared {
 
 // tm_x: hidden viewed as uint8 [T, 2H]; tm_w: hl viewed as uint8 [2 * Erows, 2H]; both with
 // 128 B x 128 row boxes and 128B swizzle (rows past the end are zero-filled by TMA).
+template <int kRowTiles>
 __global__ void __launch_bounds__(kThreads, 1)
 router_logits_tc_kernel(const __grid_constant__ CUtensorMap tm_x, const __grid_constant__ CUtensorMap tm_w,
                         float* __restrict__ logits, int T, int H, int E, int Erows, int* err) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  constexpr int kStageBytes = Cfg<kRowTiles>::kStageBytes, kWOff = kRowTiles * kABytes;
+  constexpr int kTmemCols = kRowTiles * BN;
   Shared* sh = reinterpret_cast<Shared*>(smem + kStages * kStageBytes);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int m0 = blockIdx.x * BM, n0 = blockIdx.y * BN;
+  const int m0 = blockIdx.x * (kRowTiles * BM), n0 = blockIdx.y * BN;
+  const int row_tiles = min(kRowTiles, (T - m0 + BM - 1) / BM);  // a last CTA may have one
   const int Nt = min(BN, (E - n0 + 15) / 16 * 16);  // MMA N: multiple of 16
   const int nbox = (Nt + 127) / 128;
   const int num_kb = (2 * H) / BKB;
@@ -72,7 +83,7 @@ router_logits_tc_kernel(const __grid_constant__ CUtensorMap tm_x, const __grid_c
     sh->dead = 0;
     ptx::fence_mbar_init();
   }
-  if (warp == 5) ptx::tmem_alloc<BN>(&sh->tmem_base);
+  if (warp == 5) ptx::tmem_alloc<kTmemCols>(&sh->tmem_base);
   if (warp == 4 && lane == 0) { ptx::prefetch_tmap(&tm_x); ptx::prefetch_tmap(&tm_w); }
   ptx::tc_fence_before();
   __syncthreads();
@@ -87,9 +98,9 @@ router_logits_tc_kernel(const __grid_constant__ CUtensorMap tm_x, const __grid_c
       ptx::mbar_wait(&sh->empty[stage], phase ^ 1, dead, err, 11);
       if (ptx::elect_one()) {
         uint8_t* sa = smem + stage * kStageBytes;
-        uint8_t* sb = sa + kABytes;
-        ptx::mbar_arrive_expect_tx(&sh->full[stage], kABytes + 2 * nbox * kBoxBytes);
-        ptx::tma_load_2d(sa, &tm_x, &sh->full[stage], kb * BKB, m0);
+        uint8_t* sb = sa + kWOff;
+        ptx::mbar_arrive_expect_tx(&sh->full[stage], row_tiles * kABytes + 2 * nbox * kBoxBytes);
+        for (int rt = 0; rt < row_tiles; ++rt) ptx::tma_load_2d(sa + rt * kABytes, &tm_x, &sh->full[stage], kb * BKB, m0 + rt * BM);
         for (int b = 0; b < nbox; ++b) {
           ptx::tma_load_2d(sb + b * kBoxBytes, &tm_w, &sh->full[stage], kb * BKB, n0 + b * 128);
           ptx::tma_load_2d(sb + (2 + b) * kBoxBytes, &tm_w, &sh->full[stage], kb * BKB, Erows + n0 + b * 128);
@@ -107,13 +118,15 @@ router_logits_tc_kernel(const __grid_constant__ CUtensorMap tm_x, const __grid_c
       ptx::tc_fence_after();
       if (ptx::elect_one()) {
         const uint8_t* sa = smem + stage * kStageBytes;
-        const uint64_t adesc = ptx::umma_desc_k128(sa);
-        const uint64_t hdesc = ptx::umma_desc_k128(sa + kABytes);
-        const uint64_t ldesc = ptx::umma_desc_k128(sa + kABytes + 2 * kBoxBytes);
+        const uint64_t hdesc = ptx::umma_desc_k128(sa + kWOff);
+        const uint64_t ldesc = ptx::umma_desc_k128(sa + kWOff + 2 * kBoxBytes);
+        for (int rt = 0; rt < row_tiles; ++rt) {
+          const uint64_t adesc = ptx::umma_desc_k128(sa + rt * kABytes);
 #pragma unroll
-        for (int k4 = 0; k4 < BKB / 32; ++k4) {  // UMMA_K = 16 bf16 = 32 B per step
-          ptx::umma_bf16(tmem_base, adesc + 2 * k4, hdesc + 2 * k4, idesc, (kb | k4) > 0);
-          ptx::umma_bf16(tmem_base, adesc + 2 * k4, ldesc + 2 * k4, idesc, 1);
+          for (int k4 = 0; k4 < BKB / 32; ++k4) {  // UMMA_K = 16 bf16 = 32 B per step
+            ptx::umma_bf16(tmem_base + rt * BN, adesc + 2 * k4, hdesc + 2 * k4, idesc, (kb | k4) > 0);
+            ptx::umma_bf16(tmem_base + rt * BN, adesc + 2 * k4, ldesc + 2 * k4, idesc, 1);
+          }
         }
         ptx::umma_commit(&sh->empty[stage]);
         if (kb == num_kb - 1) ptx::umma_commit(&sh->tmem_full);
@@ -124,8 +137,9 @@ router_logits_tc_kernel(const __grid_constant__ CUtensorMap tm_x, const __grid_c
   } else {
     ptx::mbar_wait(&sh->tmem_full, 0, dead, err, 13);
     ptx::tc_fence_after();
-    const int t = m0 + warp * 32 + lane;
-    const uint32_t tb = tmem_base + (static_cast<uint32_t>(warp * 32) << 16);
+   for (int rt = 0; rt < row_tiles; ++rt) {
+    const int t = m0 + rt * BM + warp * 32 + lane;
+    const uint32_t tb = tmem_base + (static_cast<uint32_t>(warp * 32) << 16) + rt * BN;
     for (int c = 0; c < Nt; c += 16) {
       uint32_t v[16];
       ptx::tmem_ld16(tb + c, v);
@@ -144,13 +158,14 @@ router_logits_tc_kernel(const __grid_constant__ CUtensorMap tm_x, const __grid_c
         }
       }
     }
+   }
   }
 
   ptx::tc_fence_before();
   __syncthreads();
   if (warp == 5) {
     ptx::tc_fence_after();
-    ptx::tmem_dealloc<BN>(tmem_base);
+    ptx::tmem_dealloc<kTmemCols>(tmem_base);
   }
 }
 

@@ -631,9 +631,15 @@ slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t
       CUtensorMap tm_x;
       slp_status st = make_tmap_u8(&tm_x, const_cast<void*>(hidden), static_cast<uint64_t>(H) * 2, static_cast<uint64_t>(T));
       if (st != SLP_OK) return st;
-      dim3 grid((T + slp::rtc::BM - 1) / slp::rtc::BM, (E + slp::rtc::BN - 1) / slp::rtc::BN);
-      slp::rtc::router_logits_tc_kernel<<<grid, slp::rtc::kThreads, slp::rtc::kSmemBytes, s>>>(tm_x, h->tm_rw, h->d_logits, T, H, E,
-                                                                                              h->Erows, h->d_err);
+      namespace rtc = slp::rtc;
+      const int row_tiles = (T + rtc::BM - 1) / rtc::BM, n_tiles = (E + rtc::BN - 1) / rtc::BN;
+      if (row_tiles * n_tiles > h->num_sms) {  // more than one wave of 128-token CTAs: two row tiles per CTA halve the W_r traffic
+        dim3 grid((row_tiles + 1) / 2, n_tiles);
+        rtc::router_logits_tc_kernel<2><<<grid, rtc::kThreads, rtc::Cfg<2>::kSmemBytes, s>>>(tm_x, h->tm_rw, h->d_logits, T, H, E, h->Erows, h->d_err);
+      } else {
+        dim3 grid(row_tiles, n_tiles);
+        rtc::router_logits_tc_kernel<1><<<grid, rtc::kThreads, rtc::Cfg<1>::kSmemBytes, s>>>(tm_x, h->tm_rw, h->d_logits, T, H, E, h->Erows, h->d_err);
+      }
     }
     const int warps = 8;
     const int blocks = (T + warps - 1) / warps;
@@ -945,7 +951,8 @@ slp_status slp_moe_stack_create(const slp_moe_cfg* cfg, int32_t n_layers, const 
   for (auto& e : h->ev_tail) CU_OR_BAIL(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
 
   // ---- per layer: pin (or check) the streamed weights, upload router / bias / block scales / shared expert ----
-  CU_OR_BAIL(cudaFuncSetAttribute(slp::rtc::router_logits_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::rtc::kSmemBytes));
+  CU_OR_BAIL(cudaFuncSetAttribute(slp::rtc::router_logits_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::rtc::Cfg<1>::kSmemBytes));
+  CU_OR_BAIL(cudaFuncSetAttribute(slp::rtc::router_logits_tc_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, slp::rtc::Cfg<2>::kSmemBytes));
   for (int l = 0; l < n_layers; ++l) {
     w = w_all + l;
     h->hw = *w;
