@@ -61,6 +61,46 @@ def test_stack_layers_equal_single_layer_handles_and_prefetch_accounting(layers)
         stack.close()
 
 
+def test_long_calls_launch_the_last_group_in_pieces():
+    """A call with >= 256 rows per expert copies and launches its LAST launch group in 8-expert pieces (the call then
+    ends a piece's compute, not a group's, after the last copy).  Same bytes, same kernels, same result as the resident
+    pass; in a stack the pieces apply to the layer the call loads itself, prefetched layers arrive whole."""
+    cfgs = [small_dsv3(name=f"tail_l{l}", T=2100, seed=60 + l) for l in range(2)]     # 2100 * 4 >= 256 * 32
+    Ws = [inputs.make_weights(c, device="cpu", pin=True) for c in cfgs]
+    hidden = inputs.make_hidden(cfgs[0], device="cpu").cuda()
+    cfg = cfgs[0]
+    resident = []
+    for c, W in zip(cfgs, Ws):
+        one = SlpMoeLayer(c, W, device=0)
+        try:
+            out_s = one.prefill(hidden).clone()
+            torch.cuda.synchronize()
+            st = one.stats()
+            # 1 shared-expert pair + the single 32-expert group as 4 pieces of 8
+            assert st["gemm_launches"] == 2 * (1 + 4), st
+            assert st["experts_copied"] == cfg.E and st["bytes_copied"] == cfg.E * 3 * cfg.I * cfg.H
+            one.set_residency("resident")
+            out_r = one.prefill(hidden).clone()
+            torch.cuda.synchronize()
+            assert one.stats()["gemm_launches"] == 2
+            assert torch.equal(out_s.view(torch.int16), out_r.view(torch.int16))
+            resident.append(out_r)
+        finally:
+            one.close()
+    stack = SlpMoeLayer(cfg, Ws, device=0)
+    try:
+        for rnd in range(2):
+            for l in range(2):
+                out = stack.prefill(hidden, layer=l).clone()
+                torch.cuda.synchronize()
+                st = stack.stats()
+                assert torch.equal(out.view(torch.int16), resident[l].view(torch.int16)), (rnd, l)
+                first = rnd == 0 and l == 0
+                assert st["gemm_launches"] == (2 * (1 + 4) if first else 2 * (1 + 1)), st   # prefetched layers: one whole group
+    finally:
+        stack.close()
+
+
 def test_stack_out_of_order_and_explicit_prefetch(layers):
     cfgs, Ws, hidden, singles = layers
     cfg = cfgs[0]
