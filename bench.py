@@ -53,8 +53,8 @@ WORKLOADS = {
 METRIC = "prefill tok/s per MoE layer (host-streamed FP8); resident FP8 TFLOP/s vs peak"
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE gemm_tc_kernel<0> launch from the committed
 # `ncu --set full` captures (profiles/r2_layer_ncu.md: the whole resident 32K layer in one launch;
-# profiles/r1_streamed_gemm_ncu.md: one 64-expert group of the streamed T = 4096 layer); None = not captured.
-NCU_TRAFFIC_BYTES = {"cfg2_resident": 10.55e9, "cfg1_streamed": 2.143e9}
+# profiles/r2_streamed_gemm_ncu.md: one 64-expert group of the streamed T = 4096 layer); None = not captured.
+NCU_TRAFFIC_BYTES = {"cfg2_resident": 10.55e9, "cfg1_streamed": 2.136e9}
 FP8_NOMINAL_TFLOPS = 4500.0
 
 
