@@ -3,28 +3,32 @@
 // One persistent CTA per SM works through the (128-row tile, N tile) work items of the experts of the
 // launch (one 16-byte record per tile, written by permute_scan_kernel); an otherwise idle warp takes the
 // items from a global counter, so all CTAs stay within ~gridDim consecutive items and share operands
-// through L2 (SLP_TRIAGE gemm=static: static round-robin instead).  Per
-// 128-deep K block the tensor core writes a fresh 128 x 256 fp32 partial into one of two TMEM
-// buffers; the promotion warps pull it out with tcgen05.ld and add it into fp32 register accumulators
+// through L2 (SLP_TRIAGE gemm=static: static round-robin instead).  Per 128-deep K block the tensor core
+// writes a fresh 128 x 256 fp32 partial into TMEM, as two independent 128-column halves (four half-buffers
+// in flight); the promotion warps pull it out with tcgen05.ld and add it into fp32 register accumulators
 // with one FMA per element (issued as FFMA2 pairs), scaled by  xs[row, kb] * ws[n-block, kb]
 // ("FP8 GEMM with FP32 accumulation"; "accumulate all partial dot-products
 // first and apply the scale once per block").
 //
 //   warp 8      TMA producer (one elected thread): A tile (128 rows x 128 B) + 64-row B boxes per K
 //               block into a 128B-swizzled smem ring (mbarrier full / empty)
-//   warp 9      MMA issuer (one elected thread): per K block 4 x tcgen05.mma.kind::f8f6f4 (M128 N256
-//               K32) into TMEM buffer kb mod 2; tcgen05.commit publishes the buffer and frees the stage
-//   warp 10     work scheduler (one elected thread): atomicAdd on the launch's counter -> 4-deep smem ring
-//               read by the producer, the MMA issuer and the promotion warps
+//   warp 9      MMA issuer (one elected thread): per K block and column half 4 x tcgen05.mma.kind::f8f6f4
+//               (M128 N128 K32) into TMEM half-buffer [kb mod 2][half]; tcgen05.commit publishes the
+//               half-buffer, a last commit frees the stage; its three barrier probes per K block are in
+//               flight together
+//   warp 10     work scheduler (one elected thread): atomicAdd on the launch's counter, reads the tile's
+//               record and publishes it through a 4-deep smem ring read by the producer, the MMA issuer
+//               and the promotion warps
 //   warp 11     idle (warps 8-11 donate most of their registers to the promotion warps, setmaxnreg)
 //   warps 0-7   promotion + epilogue: warp w owns TMEM lanes 32 * (w % 4).. (rows) and the 128 columns
-//               of half w / 4; 128 fp32 accumulators per thread; the TMEM buffer is handed back as
-//               soon as the last tcgen05.ld has landed, before the last FMAs
+//               of half w / 4; 128 fp32 accumulators per thread; a half-buffer is handed back as soon as
+//               the last tcgen05.ld has landed, before the last FMAs
 //
-// kPair (SLP_TRIAGE gemm=pair): a cluster of two CTAs issues ONE cta_group::2 MMA with M = 256 (two
-//   128-row tiles of the same expert) x N = 256; each CTA stages its own A tile and half of the B tile
-//   (TMA loads of both CTAs complete on the leader's mbarrier, commits are multicast to both CTAs, the
-//   peer's promotion warps release TMEM on the leader's barrier).  It moves a third less operand data
+// kPair (SLP_TRIAGE gemm=pair): a cluster of two CTAs issues cta_group::2 MMAs with M = 256 (two
+//   128-row tiles of the same expert) x N = 128 per column half; each CTA stages its own A tile and half of
+//   the B tile (CTA 0 the gate rows / CTA 1 the up rows of a gate/up tile; 64 rows of each column half of a
+//   down tile); TMA loads of both CTAs complete on the leader's mbarrier, commits are multicast to both CTAs,
+//   the peer's promotion warps release TMEM on the leader's barrier.  It moves a third less operand data
 //   per MAC from L2 and through the shared-memory port; see DESIGN.md §6.1 for where each variant stands.
 //
 // All barrier / stage addresses are 32-bit shared-window addresses computed once (ptx::launder_u32):
@@ -106,13 +110,6 @@ __device__ __forceinline__ void silu_mul_fast2(float& g0, float u0, float& g1, f
   asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a * b));
   g0 = g0 * (r * b) * u0;
   g1 = g1 * (r * a) * u1;
-}
-
-// p ? a : b as one SELP (keeps the scale bookkeeping of the K loop free of branches and copies).
-__device__ __forceinline__ float sel_f32(bool p, float a, float b) {
-  float r;
-  asm("{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %3, 0;\n\tselp.f32 %0, %1, %2, q;\n\t}" : "=f"(r) : "f"(a), "f"(b), "r"(static_cast<int>(p)));
-  return r;
 }
 
 // Correctly rounded h / s from a correctly rounded reciprocal and one residual step (Markstein):
