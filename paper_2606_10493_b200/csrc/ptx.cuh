@@ -161,35 +161,7 @@ __device__ __forceinline__ void tmem_ld_wait16(uint32_t (&v)[16]) {
                :: "memory");
 }
 
-// TMEM -> registers: this warp's 32 lanes x 32 consecutive 32-bit columns.  All tcgen05 wrappers are
-// asm volatile, so their program order (load, wait, use) is kept without tying registers together.
-__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
-  asm volatile(
-      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
-      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15,"
-      " %16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
-      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-        "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
-        "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
-        "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
-      : "r"(taddr) : "memory");
-}
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-
-// Empty statement that reads and "writes" 16 registers: placed after the issue of the next
-// tcgen05.ld it keeps `v` live across that issue, so the two loads in flight get distinct registers
-// (asm volatile statements are not reordered against each other).
-__device__ __forceinline__ void keep16(uint32_t (&v)[16]) {
-  asm volatile(""
-               : "+r"(v[0]), "+r"(v[1]), "+r"(v[2]), "+r"(v[3]), "+r"(v[4]), "+r"(v[5]), "+r"(v[6]), "+r"(v[7]),
-                 "+r"(v[8]), "+r"(v[9]), "+r"(v[10]), "+r"(v[11]), "+r"(v[12]), "+r"(v[13]), "+r"(v[14]), "+r"(v[15]));
-}
-
-// Empty statement that only READS 16 registers: keeps them live up to this point.
-__device__ __forceinline__ void use16(const uint32_t (&v)[16]) {
-  asm volatile("" :: "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]),
-                     "r"(v[8]), "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]));
-}
 
 // ---- shared-address variants -------------------------------------------------------------------
 // The hot loops keep every barrier / stage address as a 32-bit shared-window address computed once
@@ -273,14 +245,6 @@ __device__ __forceinline__ void sts_f32x2(uint32_t addr, float x, float y) {
   asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(addr), "f"(x), "f"(y) : "memory");
 }
 
-__device__ __forceinline__ float lds_f32(uint32_t addr) {
-  float r;
-  asm volatile("ld.shared.f32 %0, [%1];" : "=f"(r) : "r"(addr) : "memory");
-  return r;
-}
-__device__ __forceinline__ void sts_f32(uint32_t addr, float x) {
-  asm volatile("st.shared.f32 [%0], %1;" ::"r"(addr), "f"(x) : "memory");
-}
 __device__ __forceinline__ int4 lds_s32x4(uint32_t addr) {
   int4 r;
   asm volatile("ld.shared.v4.s32 {%0, %1, %2, %3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(addr) : "memory");
@@ -290,28 +254,10 @@ __device__ __forceinline__ void sts_s32x4(uint32_t addr, int4 v) {
   asm volatile("st.shared.v4.s32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 
-// Two fp32 FMAs in one instruction (FFMA2): (a0, a1) += (v0, v1) * (s, s).  `s2` holds the scale in
-// both halves.  Halves the issue slots of the block-scale promotion; ptxas allocates the pairs in
-// place (tcgen05.ld destinations and accumulators are consecutive even-aligned registers).
-__device__ __forceinline__ uint64_t pack2(float lo, float hi) {
-  uint64_t r;
-  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-  return r;
-}
-__device__ __forceinline__ void fma2(uint64_t& acc, uint32_t v0, uint32_t v1, uint64_t s2) {
-  asm volatile(
-      "{\n\t.reg .b64 a;\n\tmov.b64 a, {%1, %2};\n\t"
-      "fma.rn.f32x2 %0, a, %3, %0;\n\t}"
-      : "+l"(acc) : "r"(v0), "r"(v1), "l"(s2));
-}
-// Same with a scalar scale: ptxas emits the broadcast form (FFMA2 ... Rs.F32 ...), no packed copy of the scale.
-__device__ __forceinline__ void fma2s(uint64_t& acc, uint32_t v0, uint32_t v1, float s) {
-  asm volatile(
-      "{\n\t.reg .b64 a, b;\n\tmov.b64 a, {%1, %2};\n\tmov.b64 b, {%3, %3};\n\t"
-      "fma.rn.f32x2 %0, a, b, %0;\n\t}"
-      : "+l"(acc) : "r"(v0), "r"(v1), "f"(s));
-}
-// Same on two separate fp32 accumulators (the pair is formed inside the statement).
+// Two fp32 FMAs in one instruction (FFMA2): (a0, a1) += (v0, v1) * (s, s) on two separate fp32 accumulators; the pairs
+// are formed inside the statement and ptxas emits the broadcast form of the scale (FFMA2 ... Rs.F32 ...).  (With the
+// accumulators declared as 64-bit values ptxas accumulated half of them into the tcgen05.ld destination registers
+// and copied them back: 28-64 MOVs per K block.)
 __device__ __forceinline__ void fma2f(float& a0, float& a1, uint32_t v0, uint32_t v1, float s) {
   asm volatile(
       "{\n\t.reg .b64 a, b, c;\n\tmov.b64 a, {%2, %3};\n\tmov.b64 b, {%4, %4};\n\tmov.b64 c, {%0, %1};\n\t"
@@ -323,9 +269,6 @@ __device__ __forceinline__ uint32_t pack_f16x2(float lo, float hi) {
   uint32_t r;
   asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
   return r;
-}
-__device__ __forceinline__ void unpack2(uint64_t v, float& lo, float& hi) {
-  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
 }
 
 // ---- clusters / CTA pairs (cta_group::2) --------------------------------------------------------
