@@ -416,6 +416,21 @@ def main(argv=None):
     gu_bytes = n_exp_run * 2 * cfg.I * cfg.H + rows_total * (cfg.H + cfg.I) + rows_total * 4 * (cfg.H // 128 + cfg.I // 128)
     gu_flops = 2.0 * 2 * cfg.I * cfg.H * rows_total
     gu_time = mean("ms_gateup_sum") * 1e-3
+    # Streamed mode launches the (resident) shared expert apart from the routed groups: T rows against ONE expert is a
+    # tensor-bound launch however HBM-bound the routed groups are, so the roofline of the dominant kernel is taken over
+    # the routed launches and the shared-expert launch is reported beside it.
+    shared_launch = None
+    sh_time = mean("ms_gateup_shared") * 1e-3
+    if sh_time > 0 and cfg.n_shared and rows_routed > 0:
+        sh_rows = rows_total - rows_routed
+        sh_bytes = 2 * cfg.I * cfg.H + sh_rows * (cfg.H + cfg.I) + sh_rows * 4 * (cfg.H // 128 + cfg.I // 128)
+        sh_flops = 2.0 * 2 * cfg.I * cfg.H * sh_rows
+        shared_launch = {"kernel": "gemm_tc_kernel<0>, the shared expert's own launch", "rows": sh_rows, "ms": sh_time * 1e3,
+                         "tflops": sh_flops / sh_time / 1e12, "gbs": sh_bytes / sh_time / 1e9}
+        gu_bytes -= sh_bytes
+        gu_flops -= sh_flops
+        gu_time -= sh_time
+        rows_total, n_exp_run, n_pairs = rows_routed, n_exp_run - 1, max(1, n_pairs - 1)
     fp8_peak = 2.0 * (peaks["bf16_tflops"] if mode == "resident" else peaks["bf16_tflops_sustained"])
     ridge_rows = fp8_peak * 1e12 / (peaks["hbm_gbs"] * 1e9) / 2.0   # rows/expert where 2*M flop/B crosses the ridge
     tensor_bound = (rows_total / max(1, n_exp_run)) >= ridge_rows
@@ -436,12 +451,15 @@ def main(argv=None):
     roofline["traffic_launch_algorithmic_bytes"] = gu_bytes if mode == "resident" else gu_bytes * min(epl, cfg.E) / max(1, n_exp_run)
     roofline["algorithmic_bytes_per_launch"] = gu_bytes / n_pairs
     roofline["algorithmic_flops_per_launch"] = gu_flops / n_pairs
-    roofline["ms_per_launch"] = mean("ms_gateup_sum") / n_pairs
-    roofline["launches_per_step"] = st["timed_gemm_pairs"]
-    roofline["down_ms_per_launch"] = mean("ms_down_sum") / n_pairs
+    roofline["ms_per_launch"] = gu_time * 1e3 / n_pairs
+    roofline["launches_per_step"] = n_pairs
+    roofline["down_ms_per_launch"] = (mean("ms_down_sum") - (mean("ms_down_shared") if shared_launch else 0.0)) / n_pairs
     roofline["sm_mhz_during_kernel"] = mean("sm_mhz_gateup")
     roofline["down_sm_mhz_during_kernel"] = mean("sm_mhz_down")
     roofline["aggregate"] = f"mean over {len(iso)} isolated calls"
+    if shared_launch:
+        roofline["launches"] = "routed-expert launches only (the shared expert's own, tensor-bound launch is under shared_expert_launch)"
+        roofline["shared_expert_launch"] = shared_launch
 
     stage_keys = ("ms_total", "ms_route", "ms_experts", "ms_combine", "ms_copy_span", "ms_gateup_sum", "ms_down_sum")
     extra = {"tflops_per_call": flops_call * (world if par == "token" else 1) / (ms * 1e-3) / 1e12,

@@ -132,6 +132,9 @@ typedef struct {
   int32_t experts_prefetched; /* experts of the NEXT layer whose copies this call enqueued ahead (stacks) */
   int32_t layer;              /* layer of the stack the call ran */
   int64_t bytes_prefetched;   /* host -> HBM bytes of those prefetch copies (not part of bytes_copied) */
+  float ms_gateup_shared;     /* part of ms_gateup_sum spent in the shared expert's OWN launch (streamed mode launches it apart
+                                 from the routed groups; 0 when it shares a launch with routed experts) */
+  float ms_down_shared;       /* same for the down kernel */
 } slp_moe_stats;
 
 /* What create would allocate and how prefill would launch for a configuration (host arithmetic only). */

@@ -61,7 +61,8 @@ class Stats(C.Structure):
                 ("timed_gemm_pairs", C.c_int32), ("ms_gateup_sum", C.c_float), ("ms_down_sum", C.c_float),
                 ("sm_mhz_gateup", C.c_float), ("sm_mhz_down", C.c_float),
                 ("h2d_copies", C.c_int32), ("experts_from_prefetch", C.c_int32), ("experts_prefetched", C.c_int32),
-                ("layer", C.c_int32), ("bytes_prefetched", C.c_int64)]
+                ("layer", C.c_int32), ("bytes_prefetched", C.c_int64),
+                ("ms_gateup_shared", C.c_float), ("ms_down_shared", C.c_float)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_ if n != "struct_size"}

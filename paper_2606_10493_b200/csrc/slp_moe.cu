@@ -240,6 +240,7 @@ struct slp_moe_layer {
   std::vector<cudaEvent_t> ev_k;  // 3 events per expert launch pair: before gate/up, between, after down
   std::vector<cudaEvent_t> ev_tail;  // ON events of the pieces of a call's last launch group
   int ev_k_used = 0;
+  int ev_k_shared = -1;  // first event of the shared expert's own launch pair in ev_k (-1: it shares a launch with routed experts)
 };
 
 namespace {
@@ -560,6 +561,7 @@ slp_status launch_experts(L* h, cudaStream_t s, int e_begin, int e_end, int T, i
     }
     if (ev) {
       cudaEventRecord(ev[2], s);
+      if (e_begin == h->E) h->ev_k_shared = h->ev_k_used;  // the shared expert alone
       h->ev_k_used += 3;
     }
   }
@@ -618,6 +620,7 @@ slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t
   h->stats.layer = layer;
   h->stats_copy_valid = false;
   h->ev_k_used = 0;
+  h->ev_k_shared = -1;
   auto launched = [&](int n) { h->stats.kernel_launches += n; };
 
   CU_TRY(cudaMemsetAsync(h->d_clk, 0, 16 * sizeof(unsigned long long), s));
@@ -1384,7 +1387,7 @@ slp_status slp_moe_get_stats(slp_moe_layer* h, slp_moe_stats* stats) {
       CU_TRY(cudaEventSynchronize(h->ev_copy1));
       CU_TRY(cudaEventElapsedTime(&h->stats.ms_copy_span, h->ev_copy0, h->ev_copy1));
     }
-    h->stats.ms_gateup_sum = h->stats.ms_down_sum = 0.f;
+    h->stats.ms_gateup_sum = h->stats.ms_down_sum = h->stats.ms_gateup_shared = h->stats.ms_down_shared = 0.f;
     h->stats.timed_gemm_pairs = h->ev_k_used / 3;
     for (int i = 0; i + 3 <= h->ev_k_used; i += 3) {
       float a = 0.f, b = 0.f;
@@ -1392,6 +1395,10 @@ slp_status slp_moe_get_stats(slp_moe_layer* h, slp_moe_stats* stats) {
       CU_TRY(cudaEventElapsedTime(&b, h->ev_k[i + 1], h->ev_k[i + 2]));
       h->stats.ms_gateup_sum += a;
       h->stats.ms_down_sum += b;
+      if (i == h->ev_k_shared) {
+        h->stats.ms_gateup_shared = a;
+        h->stats.ms_down_shared = b;
+      }
     }
     unsigned long long clk[16] = {};
     CU_TRY(cudaMemcpy(clk, h->d_clk, sizeof clk, cudaMemcpyDeviceToHost));
