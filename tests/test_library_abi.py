@@ -34,7 +34,7 @@ def test_struct_sizes_match_header(built):
     # 20 four-byte fields / 14 pointers / see header
     assert ctypes.sizeof(binding._Cfg) == 20 * 4
     assert ctypes.sizeof(binding._HostWeights) == 14 * 8
-    assert ctypes.sizeof(binding.Stats) == 112  # ... + experts_from_prefetch, experts_prefetched, layer, (pad), bytes_prefetched
+    assert ctypes.sizeof(binding.Stats) == 120  # ... + experts_from_prefetch, experts_prefetched, layer, (pad), bytes_prefetched, ms_gateup_shared, ms_down_shared
 
 
 def test_invalid_arguments_are_reported(built):
