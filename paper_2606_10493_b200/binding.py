@@ -298,8 +298,8 @@ class SlpMoeLayer:
 
     def close(self):
         if self._h:
-            lib().slp_moe_layer_destroy(self._h)
-            self._h = C.c_void_p()
+            h, self._h = self._h, C.c_void_p()
+            _check(lib().slp_moe_layer_destroy(h))   # non-zero only under SLP_TRIAGE=guards (a canary band was written)
 
     def __del__(self):
         try:

@@ -116,10 +116,14 @@ inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
 //   gemm=static  one-CTA tcgen05 kernel with the static round-robin tile order
 //   gemm=pair    the cta_group::2 variant of the tcgen05 kernel
 //   router=fp32  router logits as plain fp32 FMAs instead of the tensor-core hi/lo split
+//   guards       every workspace buffer gets a 4 KB canary band before and after it; slp_moe_get_stats and destroy
+//                fail with SLP_ERR_CUDA if a band was written (compute-sanitizer is closed on the GPU pool);
+//                guards=selftest additionally writes one byte behind the counts buffer at create
 enum GemmImpl { kGemmTc = 0, kGemmSimt = 1, kGemmPair = 2, kGemmStatic = 3 };
 struct Triage {
   int gemm = kGemmTc;
   int router_fp32 = 0;
+  int guards = 0;
 };
 inline Triage read_triage() {
   Triage t;
@@ -130,6 +134,8 @@ inline Triage read_triage() {
   else if (v.find("gemm=static") != std::string::npos) t.gemm = kGemmStatic;
   else if (v.find("gemm=pair") != std::string::npos) t.gemm = kGemmPair;
   if (v.find("router=fp32") != std::string::npos) t.router_fp32 = 1;
+  if (v.find("guards") != std::string::npos) t.guards = 1;
+  if (v.find("guards=selftest") != std::string::npos) t.guards = 2;  // create damages one band on purpose (negative control)
   return t;
 }
 
@@ -239,6 +245,8 @@ struct slp_moe_layer {
   bool stats_copy_valid = false;
   std::vector<cudaEvent_t> ev_k;  // 3 events per expert launch pair: before gate/up, between, after down
   std::vector<cudaEvent_t> ev_tail;  // ON events of the pieces of a call's last launch group
+  struct Guarded { void* base; void* user; size_t bytes; const char* name; };
+  std::vector<Guarded> guarded;      // SLP_TRIAGE=guards: workspace allocations with canary bands
   int ev_k_used = 0;
   int ev_k_shared = -1;  // first event of the shared expert's own launch pair in ev_k (-1: it shares a launch with routed experts)
 };
@@ -246,6 +254,56 @@ struct slp_moe_layer {
 namespace {
 
 using L = slp_moe_layer;
+
+// Workspace allocation.  With SLP_TRIAGE=guards every buffer sits between two 4 KB canary bands (0xA5) that
+// check_guards() reads back: a kernel that writes outside a buffer (the usual way a tile-bookkeeping bug shows) is
+// caught without compute-sanitizer, which is closed on the GPU pool.
+constexpr size_t kGuardBytes = 4096;
+template <class T>
+cudaError_t ws_alloc(L* h, T** out, size_t bytes, const char* name) {
+  if (!h->triage.guards) return cudaMalloc(out, bytes);
+  char* base = nullptr;
+  const size_t padded = (bytes + 255) / 256 * 256;
+  cudaError_t e = cudaMalloc(&base, padded + 2 * kGuardBytes);
+  if (e != cudaSuccess) return e;
+  e = cudaMemset(base, 0xA5, padded + 2 * kGuardBytes);
+  if (e != cudaSuccess) return e;
+  *out = reinterpret_cast<T*>(base + kGuardBytes);
+  h->guarded.push_back({base, base + kGuardBytes, bytes, name});
+  return cudaSuccess;
+}
+void ws_free(L* h, void* user) {
+  if (!user) return;
+  for (auto& gd : h->guarded)
+    if (gd.user == user) { cudaFree(gd.base); gd.base = gd.user = nullptr; return; }
+  cudaFree(user);
+}
+// Reads the canary bands back; the first damaged one is reported.
+slp_status check_guards(L* h) {
+  if (!h->triage.guards) return SLP_OK;
+  std::vector<unsigned char> buf(kGuardBytes);
+  for (const auto& gd : h->guarded) {
+    if (!gd.base) continue;
+    const size_t padded = (gd.bytes + 255) / 256 * 256;
+    const char* bands[2] = {static_cast<const char*>(gd.base), static_cast<const char*>(gd.user) + padded};
+    for (int b = 0; b < 2; ++b) {
+      if (cudaMemcpy(buf.data(), bands[b], kGuardBytes, cudaMemcpyDeviceToHost) != cudaSuccess)
+        return fail(SLP_ERR_CUDA, "reading the guard band of %s failed: %s", gd.name, cudaGetErrorString(cudaGetLastError()));
+      for (size_t i = 0; i < kGuardBytes; ++i)
+        if (buf[i] != 0xA5)
+          return fail(SLP_ERR_CUDA, "guard band %s buffer %s (%zu bytes) overwritten at byte %zu", b ? "after" : "before", gd.name, gd.bytes, i);
+    }
+    // the slack between the buffer's end and the band (alignment padding) is canary too
+    if (padded > gd.bytes) {
+      const size_t n = padded - gd.bytes;
+      if (cudaMemcpy(buf.data(), static_cast<const char*>(gd.user) + gd.bytes, n, cudaMemcpyDeviceToHost) != cudaSuccess)
+        return fail(SLP_ERR_CUDA, "reading the slack of %s failed", gd.name);
+      for (size_t i = 0; i < n; ++i)
+        if (buf[i] != 0xA5) return fail(SLP_ERR_CUDA, "buffer %s (%zu bytes) overrun by %zu bytes", gd.name, gd.bytes, i + 1);
+    }
+  }
+  return SLP_OK;
+}
 
 void select_layer(L* h, int l) {
   if (h->cur_layer == l) return;
@@ -1029,28 +1087,29 @@ slp_status slp_moe_stack_create(const slp_moe_cfg* cfg, int32_t n_layers, const 
 
   // workspace
   const size_t Tm = h->Tm, rows = h->rows_max;
-  CU_OR_BAIL(cudaMalloc(&h->d_logits, Tm * E * sizeof(float)));
-  CU_OR_BAIL(cudaMalloc(&h->d_idx, Tm * k * sizeof(int32_t)));
-  CU_OR_BAIL(cudaMalloc(&h->d_w, Tm * k * sizeof(float)));
-  CU_OR_BAIL(cudaMalloc(&h->d_counts, E * sizeof(int32_t)));
-  CU_OR_BAIL(cudaMalloc(&h->d_chunk, static_cast<size_t>(h->n_chunks_max) * E * sizeof(int32_t)));
-  CU_OR_BAIL(cudaMalloc(&h->d_row_start, (E + 2) * sizeof(int32_t)));
-  CU_OR_BAIL(cudaMalloc(&h->d_tile_start, (E + 2) * sizeof(int32_t)));
-  CU_OR_BAIL(cudaMalloc(&h->d_tile_expert, static_cast<size_t>(h->tiles_max) * sizeof(int32_t)));
-  CU_OR_BAIL(cudaMalloc(&h->d_tile_info, static_cast<size_t>(h->tiles_max) * sizeof(int4)));
-  CU_OR_BAIL(cudaMalloc(&h->d_pair_start, (E + 2) * sizeof(int32_t)));
-  CU_OR_BAIL(cudaMalloc(&h->d_pair_expert, static_cast<size_t>(h->tiles_max) * sizeof(int32_t)));
-  CU_OR_BAIL(cudaMalloc(&h->d_pos, Tm * k * sizeof(int32_t)));
-  CU_OR_BAIL(cudaMalloc(&h->d_row_token, rows * sizeof(int32_t)));
-  CU_OR_BAIL(cudaMalloc(&h->d_xq, rows * H));
-  CU_OR_BAIL(cudaMalloc(&h->d_xs, rows * h->xs_stride * sizeof(float)));
-  CU_OR_BAIL(cudaMalloc(&h->d_hq, rows * I));
-  CU_OR_BAIL(cudaMalloc(&h->d_hs, rows * h->hs_stride * sizeof(float)));
-  CU_OR_BAIL(cudaMalloc(&h->d_y, rows * H * sizeof(uint16_t)));
-  CU_OR_BAIL(cudaMalloc(&h->d_ys, rows * h->ys_stride * sizeof(float)));
-  CU_OR_BAIL(cudaMalloc(&h->d_clk, 16 * sizeof(unsigned long long)));
-  CU_OR_BAIL(cudaMalloc(&h->d_sched, 2 * sizeof(int)));
-  CU_OR_BAIL(cudaMalloc(&h->d_err, sizeof(int)));
+  CU_OR_BAIL(ws_alloc(h, &h->d_logits, Tm * E * sizeof(float), "d_logits"));
+  CU_OR_BAIL(ws_alloc(h, &h->d_idx, Tm * k * sizeof(int32_t), "d_idx"));
+  CU_OR_BAIL(ws_alloc(h, &h->d_w, Tm * k * sizeof(float), "d_w"));
+  CU_OR_BAIL(ws_alloc(h, &h->d_counts, E * sizeof(int32_t), "d_counts"));
+  CU_OR_BAIL(ws_alloc(h, &h->d_chunk, static_cast<size_t>(h->n_chunks_max) * E * sizeof(int32_t), "d_chunk"));
+  CU_OR_BAIL(ws_alloc(h, &h->d_row_start, (E + 2) * sizeof(int32_t), "d_row_start"));
+  CU_OR_BAIL(ws_alloc(h, &h->d_tile_start, (E + 2) * sizeof(int32_t), "d_tile_start"));
+  CU_OR_BAIL(ws_alloc(h, &h->d_tile_expert, static_cast<size_t>(h->tiles_max) * sizeof(int32_t), "d_tile_expert"));
+  CU_OR_BAIL(ws_alloc(h, &h->d_tile_info, static_cast<size_t>(h->tiles_max) * sizeof(int4), "d_tile_info"));
+  CU_OR_BAIL(ws_alloc(h, &h->d_pair_start, (E + 2) * sizeof(int32_t), "d_pair_start"));
+  CU_OR_BAIL(ws_alloc(h, &h->d_pair_expert, static_cast<size_t>(h->tiles_max) * sizeof(int32_t), "d_pair_expert"));
+  CU_OR_BAIL(ws_alloc(h, &h->d_pos, Tm * k * sizeof(int32_t), "d_pos"));
+  CU_OR_BAIL(ws_alloc(h, &h->d_row_token, rows * sizeof(int32_t), "d_row_token"));
+  CU_OR_BAIL(ws_alloc(h, &h->d_xq, rows * H, "d_xq"));
+  CU_OR_BAIL(ws_alloc(h, &h->d_xs, rows * h->xs_stride * sizeof(float), "d_xs"));
+  CU_OR_BAIL(ws_alloc(h, &h->d_hq, rows * I, "d_hq"));
+  CU_OR_BAIL(ws_alloc(h, &h->d_hs, rows * h->hs_stride * sizeof(float), "d_hs"));
+  CU_OR_BAIL(ws_alloc(h, &h->d_y, rows * H * sizeof(uint16_t), "d_y"));
+  CU_OR_BAIL(ws_alloc(h, &h->d_ys, rows * h->ys_stride * sizeof(float), "d_ys"));
+  CU_OR_BAIL(ws_alloc(h, &h->d_clk, 16 * sizeof(unsigned long long), "d_clk"));
+  CU_OR_BAIL(ws_alloc(h, &h->d_sched, 2 * sizeof(int), "d_sched"));
+  CU_OR_BAIL(ws_alloc(h, &h->d_err, sizeof(int), "d_err"));
+  if (h->triage.guards == 2) CU_OR_BAIL(cudaMemset(reinterpret_cast<char*>(h->d_counts + E), 0, 1));  // negative control of the canary check
   CU_OR_BAIL(cudaMemset(h->d_err, 0, sizeof(int)));
   CU_OR_BAIL(cudaMemset(h->d_tile_expert, 0, static_cast<size_t>(h->tiles_max) * sizeof(int32_t)));
   CU_OR_BAIL(cudaMemset(h->d_tile_info, 0, static_cast<size_t>(h->tiles_max) * sizeof(int4)));
@@ -1265,6 +1324,7 @@ slp_status slp_moe_layer_destroy(slp_moe_layer* h) {
   if (!h) return SLP_OK;
   cudaSetDevice(h->cfg.device);
   cudaDeviceSynchronize();
+  const slp_status guard_status = check_guards(h);  // reported by destroy too (SLP_TRIAGE=guards)
   free_pool(h);
   if (h->cur_layer >= 0 && h->cur_layer < static_cast<int>(h->layers.size())) stash_layer(h, h->cur_layer);
   for (LayerW& w : h->layers) {
@@ -1275,8 +1335,7 @@ slp_status slp_moe_layer_destroy(slp_moe_layer* h) {
   void* ptrs[] = {h->d_logits, h->d_w, h->d_xs, h->d_hs, h->d_idx,
                   h->d_counts, h->d_chunk, h->d_row_start, h->d_tile_start, h->d_tile_expert, h->d_pair_start, h->d_pair_expert, h->d_tile_info, h->d_pos, h->d_row_token, h->d_xq,
                   h->d_hq, h->d_y, h->d_ys, h->d_err, h->d_clk, h->d_sched, h->d_e2e_in, h->d_e2e_out};
-  for (void* p : ptrs)
-    if (p) cudaFree(p);
+  for (void* p : ptrs) ws_free(h, p);
   if (h->h_counts) cudaFreeHost(h->h_counts);
   if (h->h_err) cudaFreeHost(h->h_err);
   for (void* p : h->registered) unregister_host_range(p);
@@ -1293,7 +1352,7 @@ slp_status slp_moe_layer_destroy(slp_moe_layer* h) {
     if (e) cudaEventDestroy(e);
   cudaGetLastError();
   delete h;
-  return SLP_OK;
+  return guard_status;
 }
 
 slp_status slp_moe_debug_routing(slp_moe_layer* h, int32_t* idx, float* w, int32_t* counts) {
@@ -1416,6 +1475,8 @@ slp_status slp_moe_get_stats(slp_moe_layer* h, slp_moe_stats* stats) {
   }
   *stats = h->stats;
   stats->struct_size = sizeof(slp_moe_stats);
+  slp_status gst = check_guards(h);
+  if (gst != SLP_OK) return gst;
   return check_kernel_error(h);
 }
 
