@@ -210,6 +210,29 @@ def test_cfg2_32k_resident_streamed_chunked(dsv3):
         layer.close()
 
 
+def test_cfg2_resident_soak_is_bitwise_stable(dsv3):
+    """120 back-to-back resident 32K-token calls (the chip settles under its power cap, clocks move, CTAs take
+    different tiles from the dynamic scheduler every time): every output equals the first bit for bit, the
+    in-kernel watchdog never fires.  A hand-off race in the GEMM pipeline would show here as a flipped output."""
+    W, _ = dsv3
+    cfg = inputs.CONFIGS[2]
+    hidden = inputs.make_hidden(cfg, device=torch.device("cuda", 0))
+    layer = SlpMoeLayer(cfg, W, device=0)
+    try:
+        layer.set_residency("resident")
+        first = layer.prefill(hidden).clone()
+        torch.cuda.synchronize()
+        out = torch.empty_like(first)
+        for i in range(120):
+            layer.prefill(hidden, out=out)
+            if i % 10 == 9:
+                torch.cuda.synchronize()
+                assert torch.equal(out.view(torch.int16), first.view(torch.int16)), f"call {i} differs from the first"
+        layer.stats()   # raises if a pipeline wait timed out
+    finally:
+        layer.close()
+
+
 def test_cfg2_cta_pair_kernel_full_size(dsv3):
     """The cta_group::2 variant (SLP_TRIAGE gemm=pair) at full size: resident 32K pass against the oracle on
     the tile-boundary tokens, and streamed with empty launch groups impossible here but 64-expert groups."""
