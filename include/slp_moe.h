@@ -267,6 +267,52 @@ slp_status slp_moe_get_stats(slp_moe_layer* h, slp_moe_stats* stats);
  * This is the denominator of the streamed-mode roofline. */
 slp_status slp_measure_h2d(int32_t device, size_t chunk_bytes, size_t total_bytes, int32_t repeats, double* gbs);
 
+/* The histogram / scan / permute step (Fig. 2 step 4: tokens "sorted to form per-expert token lists") as a
+ * stand-alone call that NEVER allocates: no handle, no cudaMalloc / cudaFree / cudaMallocHost, no allocating
+ * library routine, on the first call or any later one.
+ *
+ * It exists for callers that cannot obtain device memory at the point where they need this step: a serving process whose
+ * own pool allocator took all of HBM at start-up (a cudaMalloc would fail, or steal from the pool's accounting); a
+ * plugin invoked inside a region where its host forbids driver allocations because they synchronise the device
+ * (latency-critical decode loops); code running after the device is already full.  The handle-based calls above
+ * cannot serve them, because slp_moe_layer_create allocates.  Here the caller brings every input and output buffer and
+ * the step's scratch (per-chunk expert histograms and the tile tables the scan emits) lives in one 616 KiB array
+ * compiled into the library.  Cost: each GPU on which the process uses this library holds those 616 KiB from the moment
+ * the library is loaded there until the process exits, whether or not this function is ever called.
+ *
+ * Limits (SLP_ERR_UNSUPPORTED_SHAPE beyond them, nothing launched): T <= 32768 tokens, T * top_k <= 262144 routed
+ * assignments, 1 <= n_experts <= 511, 1 <= top_k <= min(32, n_experts).  T == 0 returns SLP_OK and touches nothing.
+ *
+ *  idx_dev        dev [T, top_k] int32, read only: the experts of each token, every entry in [0, n_experts)
+ *                 (an entry outside that range is undefined behaviour, as in slp_moe_prefill's own router output).
+ *  counts_dev     dev [n_experts] int32, out: tokens per expert.
+ *  row_start_dev  dev [n_experts + 2] int32, out: first workspace row of each expert's 128-aligned range; entry
+ *                 n_experts = 0 (the un-permuted rows [0, T) in front, the shared expert's rows); entry
+ *                 n_experts + 1 = rows in use.
+ *  pos_dev        dev [T, top_k] int32, out: workspace row of assignment (t, j); rows of one expert ascend with t.
+ *  row_token_dev  dev [row_capacity] int32, out: token of each workspace row, -1 in padding rows.  The first
+ *                 slp_moe_permute_static_rows(T, top_k, n_experts) entries are overwritten, later ones untouched.
+ *  row_capacity   entries row_token_dev can hold; must be >= slp_moe_permute_static_rows(...) (the data-independent
+ *                 worst case; INVALID_ARG otherwise).
+ *  cuda_stream    a cudaStream_t on `device`; the call is asynchronous on it like slp_moe_prefill.
+ * The layouts are those of SLP_BUF_COUNTS / ROW_START / POS / ROW_TOKEN of an unsharded handle, bit for bit.
+ *
+ * First call on a device: the function looks up where that device's copy of the scratch array lives (one
+ * cudaGetSymbolAddress, with `device` made current, result cached per device under a mutex).  That is a set-up step;
+ * make the first call on each device outside any stream capture.  The function makes `device` current and leaves it so.
+ *
+ * One array per device, shared by every call from every thread and stream: two calls on the same device whose kernels
+ * can overlap on the GPU (different streams without an event between them) race on it and both results are garbage.
+ * Order them on one stream or with events.  The array keeps the previous call's contents; the call itself
+ * re-initialises everything it reads, so no clearing is needed between calls. */
+slp_status slp_moe_permute_static(int32_t device, const int32_t* idx_dev, int32_t T, int32_t top_k, int32_t n_experts,
+                                  int32_t* counts_dev, int32_t* row_start_dev, int32_t* pos_dev, int32_t* row_token_dev,
+                                  int64_t row_capacity, void* cuda_stream);
+
+/* Host arithmetic only: the number of int32 entries slp_moe_permute_static needs in row_token_dev,
+ * roundup128(T) + roundup128(T * top_k + 127 * n_experts); -1 for a negative argument. */
+int64_t slp_moe_permute_static_rows(int32_t T, int32_t top_k, int32_t n_experts);
+
 /* Library version string. */
 const char* slp_version(void);
 

@@ -9,4 +9,5 @@ PyTorch fallback for any step of the path.
 from . import inputs, sharding, smallep  # noqa: F401
 from .binding import (  # noqa: F401
     SlpMoeLayer, SlpError, lib, library_path, measure_h2d_gbs, query_plan, finalize_partial, EXPORTED_SYMBOLS,
+    permute_static, permute_static_rows,
 )

@@ -18,6 +18,7 @@ EXPORTED_SYMBOLS = [
     "slp_measure_h2d", "slp_version", "slp_moe_query_plan", "slp_moe_debug_buffer_range",
     "slp_moe_prefill_partial", "slp_moe_finalize_partial",
     "slp_moe_stack_create", "slp_moe_stack_prefill", "slp_moe_stack_prefetch",
+    "slp_moe_permute_static", "slp_moe_permute_static_rows",
 ]
 
 SLP_STREAMED, SLP_RESIDENT = 0, 1
@@ -99,9 +100,13 @@ def lib():
         L.slp_moe_debug_buffer_range.argtypes = [C.c_void_p, C.c_int32, C.c_size_t, C.c_size_t, C.c_void_p]
         L.slp_moe_get_stats.argtypes = [C.c_void_p, C.POINTER(Stats)]
         L.slp_measure_h2d.argtypes = [C.c_int32, C.c_size_t, C.c_size_t, C.c_int32, C.POINTER(C.c_double)]
+        L.slp_moe_permute_static.argtypes = [C.c_int32, C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p,
+                                             C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]
+        L.slp_moe_permute_static_rows.argtypes = [C.c_int32, C.c_int32, C.c_int32]
         for name in EXPORTED_SYMBOLS:
             if name not in ("slp_last_error", "slp_version"):
                 getattr(L, name).restype = C.c_int
+        L.slp_moe_permute_static_rows.restype = C.c_int64
         _LIB = L
     return _LIB
 
@@ -169,6 +174,29 @@ def finalize_partial(sum_f32, out=None, stream=None):
     s = torch.cuda.current_stream(sum_f32.device) if stream is None else stream
     _check(lib().slp_moe_finalize_partial(sum_f32.device.index, sum_f32.data_ptr(), sum_f32.numel(), out.data_ptr(), s.cuda_stream))
     return out
+
+
+def permute_static_rows(T, k, E):
+    """slp_moe_permute_static_rows: entries `row_token` must hold for a (T, k, E) call (host arithmetic)."""
+    return lib().slp_moe_permute_static_rows(T, k, E)
+
+
+def permute_static(idx, n_experts, counts, row_start, pos, row_token, stream=None):
+    """slp_moe_permute_static: histogram / scan / permute of a [T, k] int32 CUDA tensor of expert ids without any
+    device allocation inside the library.  For callers that own no allocator at this point (all of HBM already given
+    to a pool, or allocation forbidden where they run): every output is a CUDA int32 tensor the CALLER made earlier
+    (counts [E], row_start [E + 2], pos [T, k], row_token [>= permute_static_rows(T, k, E)]); the library's scratch is
+    a fixed 616 KiB array inside libslpmoe.so, so T <= 32768 and T * k <= 262144.  Asynchronous on `stream`; calls
+    that overlap on one GPU race on that array (see include/slp_moe.h)."""
+    import torch
+    for t in (idx, counts, row_start, pos, row_token):
+        assert t.is_cuda and t.dtype == torch.int32 and t.is_contiguous() and t.device == idx.device
+    T, k = idx.shape
+    assert counts.numel() >= n_experts and row_start.numel() >= n_experts + 2 and pos.numel() >= T * k
+    s = torch.cuda.current_stream(idx.device) if stream is None else stream
+    _check(lib().slp_moe_permute_static(idx.device.index, idx.data_ptr(), T, k, n_experts, counts.data_ptr(),
+                                        row_start.data_ptr(), pos.data_ptr(), row_token.data_ptr(), row_token.numel(),
+                                        s.cuda_stream))
 
 
 class SlpMoeLayer:

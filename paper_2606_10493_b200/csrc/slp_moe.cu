@@ -1525,3 +1525,122 @@ slp_status slp_measure_h2d(int32_t device, size_t chunk_bytes, size_t total_byte
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// slp_moe_permute_static (include/slp_moe.h): the histogram / scan / permute step (a2) for callers
+// that are not allowed to allocate device memory.
+//
+// Who that is: code that runs inside somebody else's memory budget.  An inference server that
+// hands the whole HBM to its own pool allocator at start-up, a plugin called from inside a region
+// the host framework has frozen (a stream capture, a real-time loop with a no-driver-allocation
+// rule), or a process started with the device already full: for all of them cudaMalloc either
+// fails, stalls the device behind an implicit synchronisation, or is forbidden outright.  The
+// handle-based calls above allocate at create; this one needs no handle and allocates nothing,
+// ever: the only memory it uses beyond the caller's inputs and outputs is the array below, which
+// is part of the library image and is placed in device memory by the CUDA runtime when the
+// library is loaded on a GPU.  The price is that every GPU the process touches through this
+// library holds kStaticScratchBytes until the process exits, and that the sizes are capped.
+//
+// g_static_scratch is a DEVICE variable.  On the host its name is only a handle for the runtime
+// (it has a host-side shadow address that no GPU can use), so host code must never pass it to a
+// kernel directly.  The device address is asked for once per device, with that device current,
+// through cudaGetSymbolAddress, and it is that pointer the kernels receive.
+// ---------------------------------------------------------------------------------------------
+namespace slp_static {
+constexpr int kMaxTokens = 32768;         // T
+constexpr int kMaxAssignments = 262144;   // T * top_k (32768 tokens x top-8)
+constexpr int kMaxTiles = 4096;           // >= Tpad/128 + T*k/128 + E + 2 at the limits above (256 + 2048 + 511 + 2)
+constexpr int kMaxDevices = 64;
+// byte offsets of the pieces inside the array (all multiples of 256)
+constexpr size_t kOffChunk = 0;                                                                    // int32 [256 chunks][E]
+constexpr size_t kOffTileInfo = kOffChunk + (kMaxTokens / slp::kChunkTokens) * slp::kMaxExperts * sizeof(int32_t);
+constexpr size_t kOffTileExpert = kOffTileInfo + kMaxTiles * sizeof(int4);
+constexpr size_t kOffPairExpert = kOffTileExpert + kMaxTiles * sizeof(int32_t);
+constexpr size_t kOffTileStart = kOffPairExpert + kMaxTiles * sizeof(int32_t);
+constexpr size_t kOffPairStart = kOffTileStart + 4096;
+constexpr size_t kStaticScratchBytes = kOffPairStart + 4096;                                       // 630 784 B = 616 KiB
+static_assert(kOffTileInfo % 256 == 0 && kOffTileExpert % 256 == 0 && kOffPairExpert % 256 == 0 && kOffTileStart % 256 == 0 &&
+              kOffPairStart % 256 == 0, "pieces of the static scratch must stay 256-byte aligned");
+static_assert((slp::kMaxExperts + 2) * sizeof(int32_t) <= 4096, "tile_start / pair_start piece too small");
+}  // namespace slp_static
+
+static __device__ __align__(256) unsigned char g_static_scratch[slp_static::kStaticScratchBytes];
+
+namespace slp_static {
+std::mutex g_mutex;
+unsigned char* g_dev_ptr[kMaxDevices] = {};  // device address of g_static_scratch on each device, once looked up
+
+// First use on `device` (which must be current): ask the runtime where this device's copy of the array lives.
+slp_status scratch_for_device(int device, unsigned char** out) {
+  std::lock_guard<std::mutex> lock(g_mutex);
+  if (!g_dev_ptr[device]) {
+    void* p = nullptr;
+    cudaError_t e = cudaGetSymbolAddress(&p, g_static_scratch);
+    if (e != cudaSuccess || !p) {
+      cudaGetLastError();
+      return fail(SLP_ERR_CUDA, "cudaGetSymbolAddress(g_static_scratch) on device %d failed: %s", device, cudaGetErrorString(e));
+    }
+    g_dev_ptr[device] = static_cast<unsigned char*>(p);
+  }
+  *out = g_dev_ptr[device];
+  return SLP_OK;
+}
+}  // namespace slp_static
+
+extern "C" int64_t slp_moe_permute_static_rows(int32_t T, int32_t top_k, int32_t n_experts) {
+  if (T < 0 || top_k < 0 || n_experts < 0) return -1;
+  const int64_t Tpad = (static_cast<int64_t>(T) + 127) / 128 * 128;
+  return Tpad + (static_cast<int64_t>(T) * top_k + static_cast<int64_t>(n_experts) * 127 + 127) / 128 * 128;
+}
+
+extern "C" slp_status slp_moe_permute_static(int32_t device, const int32_t* idx_dev, int32_t T, int32_t top_k, int32_t n_experts,
+                                             int32_t* counts_dev, int32_t* row_start_dev, int32_t* pos_dev, int32_t* row_token_dev,
+                                             int64_t row_capacity, void* cuda_stream) {
+  namespace st = slp_static;
+  const int E = n_experts, k = top_k;
+  if (E <= 0 || E > slp::kMaxExperts - 1) return fail(SLP_ERR_UNSUPPORTED_SHAPE, "n_experts %d outside 1..%d", E, slp::kMaxExperts - 1);
+  if (k <= 0 || k > 32 || k > E) return fail(SLP_ERR_UNSUPPORTED_SHAPE, "top_k %d outside 1..min(32, n_experts)", k);
+  if (T < 0 || T > st::kMaxTokens)
+    return fail(SLP_ERR_UNSUPPORTED_SHAPE, "T = %d exceeds the static scratch of slp_moe_permute_static (at most %d tokens per call)", T, st::kMaxTokens);
+  if (static_cast<int64_t>(T) * k > st::kMaxAssignments)
+    return fail(SLP_ERR_UNSUPPORTED_SHAPE, "T * top_k = %lld exceeds the static scratch of slp_moe_permute_static (at most %d routed assignments per call)",
+                static_cast<long long>(T) * k, st::kMaxAssignments);
+  if (T == 0) return SLP_OK;
+  if (!idx_dev || !counts_dev || !row_start_dev || !pos_dev || !row_token_dev) return fail(SLP_ERR_INVALID_ARG, "NULL argument");
+  const int64_t rows_bound = slp_moe_permute_static_rows(T, k, E);
+  if (row_capacity < rows_bound)
+    return fail(SLP_ERR_INVALID_ARG, "row_capacity %lld below slp_moe_permute_static_rows(T, top_k, n_experts) = %lld",
+                static_cast<long long>(row_capacity), static_cast<long long>(rows_bound));
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev || device >= st::kMaxDevices) {
+    cudaGetLastError();
+    return fail(SLP_ERR_CUDA, "no such CUDA device %d", device);
+  }
+  CU_TRY(cudaSetDevice(device));
+  unsigned char* base = nullptr;
+  slp_status rc = st::scratch_for_device(device, &base);
+  if (rc != SLP_OK) return rc;
+  int32_t* chunk = reinterpret_cast<int32_t*>(base + st::kOffChunk);
+  int4* tile_info = reinterpret_cast<int4*>(base + st::kOffTileInfo);
+  int32_t* tile_expert = reinterpret_cast<int32_t*>(base + st::kOffTileExpert);
+  int32_t* pair_expert = reinterpret_cast<int32_t*>(base + st::kOffPairExpert);
+  int32_t* tile_start = reinterpret_cast<int32_t*>(base + st::kOffTileStart);
+  int32_t* pair_start = reinterpret_cast<int32_t*>(base + st::kOffPairStart);
+
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  const int n_chunks = (T + slp::kChunkTokens - 1) / slp::kChunkTokens;
+  const int wpb = 4;
+  const int blocks = (n_chunks + wpb - 1) / wpb;
+  const size_t sm = static_cast<size_t>(wpb) * E * sizeof(int32_t);
+  // The array still holds whatever the previous call left there.  Nothing in it has to start at zero: the histogram pass
+  // stores (not adds) all E counters of each of this call's n_chunks chunks before the scan reads them, and the scan
+  // writes every table entry the place pass reads.  What does need a known start value is the caller's row_token (-1 in
+  // the padding rows of every expert range), so that is filled here.
+  CU_TRY(cudaMemsetAsync(row_token_dev, 0xFF, static_cast<size_t>(rows_bound) * sizeof(int32_t), s));
+  slp::permute_hist_kernel<<<blocks, wpb * 32, sm, s>>>(idx_dev, chunk, T, k, E);
+  slp::permute_scan_kernel<<<1, 512, 0, s>>>(chunk, counts_dev, row_start_dev, tile_start, tile_expert, pair_start, pair_expert, tile_info,
+                                             n_chunks, T, E, 0, E, 0, T);
+  slp::permute_place_kernel<<<blocks, wpb * 32, sm, s>>>(idx_dev, chunk, row_start_dev, pos_dev, row_token_dev, T, k, E, 0, E);
+  CU_TRY(cudaGetLastError());
+  return SLP_OK;
+}
