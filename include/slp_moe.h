@@ -231,7 +231,9 @@ slp_status slp_moe_prefill(slp_moe_layer* h, const void* hidden_bf16, int32_t T,
  *  hidden_bf16: dev [T, H], the ALL-GATHERED hidden states of all ranks (same on every rank).
  *  partial_f32: dev [T, H] fp32, fully overwritten with  sum over this handle's experts of w[t,j] * FFN(hidden[t])
  *  for every token, plus FFN_shared(hidden[t]) for tokens t in [shared_token_begin, shared_token_end) only (the
- *  shared expert is token-sharded; an empty range leaves it out).  No bf16 rounding: the ranks' partial sums are
+ *  shared expert is token-sharded; an empty range leaves it out; the range may start and end at any token: internally
+ *  the shared expert's GEMMs start at shared_token_begin rounded down to a multiple of 32, which is what
+ *  SLP_BUF_ROW_START[E] then reports, and the extra rows are never added to anything).  No bf16 rounding: the ranks' partial sums are
  *  added first (reduce-scatter) and rounded once by slp_moe_finalize_partial.  Works on an unsharded handle too
  *  (then the partial sum is the whole layer in fp32).  Ordering, copy stream and error rules as slp_moe_prefill. */
 slp_status slp_moe_prefill_partial(slp_moe_layer* h, const void* hidden_bf16, int32_t T, float* partial_f32,

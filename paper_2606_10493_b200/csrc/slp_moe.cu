@@ -669,7 +669,14 @@ slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t
   if (sh_t1 < 0) sh_t1 = T;
   if (h->cfg.n_shared == 0) sh_t0 = sh_t1 = 0;
   const bool shared = sh_t1 > sh_t0;
-  h->sh_rows = sh_t1 - sh_t0;
+  // The GEMMs run the shared expert over rows [sh_g0, sh_t1), sh_g0 = sh_t0 rounded down to a multiple of 32: the down
+  // kernel stores Y / ys in whole 32-row groups counted from the range's first row, so a range that starts on a group
+  // boundary ends its last group at roundup32(sh_t1) <= Tpad and cannot spill into the first routed expert's rows
+  // (an arbitrary start could, by up to 31 rows, when sh_t1 is within 31 rows of Tpad).  The up to 31 extra rows in
+  // front hold other tokens' quantised hidden states (quant_scatter writes every token's own row), their Y rows are
+  // computed and never read: the combine kernel keeps the caller's [sh_t0, sh_t1).
+  const int sh_g0 = shared ? (sh_t0 & ~31) : sh_t0;
+  h->sh_rows = sh_t1 - sh_g0;
   const int e_own0 = h->e0, e_own1 = h->e1;
   h->stats = slp_moe_stats{};
   h->stats.struct_size = sizeof(slp_moe_stats);
@@ -742,7 +749,7 @@ slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t
     CU_TRY(cudaMemsetAsync(h->d_row_token, 0xFF, static_cast<size_t>(h->rows_max) * sizeof(int32_t), s));
     slp::permute_hist_kernel<<<blocks, wpb * 32, sm, s>>>(h->d_idx, h->d_chunk, T, k, E);
     slp::permute_scan_kernel<<<1, 512, 0, s>>>(h->d_chunk, h->d_counts, h->d_row_start, h->d_tile_start, h->d_tile_expert, h->d_pair_start, h->d_pair_expert, h->d_tile_info, n_chunks, T,
-                                               E, e_own0, e_own1, sh_t0, sh_t1);
+                                               E, e_own0, e_own1, sh_g0, sh_t1);
     slp::permute_place_kernel<<<blocks, wpb * 32, sm, s>>>(h->d_idx, h->d_chunk, h->d_row_start, h->d_pos, h->d_row_token, T, k, E, e_own0, e_own1);
     launched(3);
   }

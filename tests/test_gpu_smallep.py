@@ -10,7 +10,11 @@ import torch
 
 from oracle.acceptance import compare_routing, compare_output
 from paper_2606_10493_b200 import SlpMoeLayer, SlpError, finalize_partial, inputs, sharding, smallep
-from test_gpu_parity import problem
+from test_gpu_parity import problem, CASES, small_dsv3
+
+# T = 1020 (Tpad = 1024) over 3 ranks: the last rank's shared-expert token range is [680, 1020), which neither starts
+# on a 32-row boundary nor ends more than 31 rows before Tpad (the 32-row output groups of the down kernel)
+CASES["mini_dsv3_1020"] = small_dsv3(name="mini_dsv3_1020", T=1020, seed=15)
 
 pytestmark = pytest.mark.gpu
 
@@ -25,8 +29,8 @@ def close_to_single_gpu(out, out_single):
     return ok, float((a != b).float().mean())
 
 
-@pytest.mark.parametrize("name", ["mini_dsv3_ragged", "mini_zipf", "mini_softmax"])
-@pytest.mark.parametrize("G", [2, 4])
+@pytest.mark.parametrize("name,G", [(n, G) for n in ("mini_dsv3_ragged", "mini_zipf", "mini_softmax") for G in (2, 4)] +
+                         [("mini_dsv3_1020", 3)])
 @pytest.mark.parametrize("mode", ["resident", "streamed"])
 def test_emulated_ranks_match_single_gpu(name, G, mode):
     cfg, W, hidden, ref = problem(name)
@@ -68,6 +72,30 @@ def test_emulated_ranks_match_single_gpu(name, G, mode):
     assert o["passed"], o
     ok, frac = close_to_single_gpu(out, out_single)
     assert ok and frac < 2e-2, frac
+
+
+@pytest.mark.parametrize("mode", ["resident", "streamed"])
+@pytest.mark.parametrize("rng", [(997, 1020), (1, 1020), (33, 34), (680, 1020), (1019, 1020)])
+def test_arbitrary_shared_token_range_on_an_unsharded_handle(mode, rng):
+    """The shared expert over [t0, t1) for ranges that start anywhere: tokens inside get exactly the full layer's fp32
+    sum, tokens outside exactly the routed-only sum (the routed rows next to the shared region stay intact)."""
+    cfg, W, hidden, _ = problem("mini_dsv3_1020")
+    x = hidden.cuda()
+    layer = SlpMoeLayer(cfg, W, device=0)
+    try:
+        layer.set_residency(mode)
+        whole = layer.prefill_partial(x, shared_tokens=(0, cfg.T)).clone()
+        routed = layer.prefill_partial(x, shared_tokens=(0, 0)).clone()
+        part = layer.prefill_partial(x, shared_tokens=rng).clone()
+        torch.cuda.synchronize()
+        row_start = layer.debug_buffer("row_start", np.int32)
+    finally:
+        layer.close()
+    t0, t1 = rng
+    assert torch.equal(part[t0:t1], whole[t0:t1])
+    assert torch.equal(part[:t0], routed[:t0]) and torch.equal(part[t1:], routed[t1:])
+    assert not torch.equal(whole[t0:t1], routed[t0:t1])
+    assert row_start[cfg.E] == t0 // 32 * 32
 
 
 def test_world_size_one_runner_equals_prefill():
