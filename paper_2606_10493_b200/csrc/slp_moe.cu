@@ -445,13 +445,14 @@ slp_status alloc_pool(L* h, int n_stage, int epl) {
 // borrow the SAME host weight copy (prefill and decode share one resident DRAM copy, zero-copy), and
 // the range must stay page-locked until the last of them is destroyed.
 std::mutex g_reg_mutex;
-std::map<void*, int> g_registered;
+struct Registered { int refs; size_t bytes; };
+std::map<void*, Registered> g_registered;  // start of each range this library registered -> users, length
 
 void unregister_host_range(void* p) {
   std::lock_guard<std::mutex> lock(g_reg_mutex);
   auto it = g_registered.find(p);
   if (it == g_registered.end()) return;
-  if (--it->second == 0) {
+  if (--it->second.refs == 0) {
     cudaHostUnregister(p);
     g_registered.erase(it);
   }
@@ -479,31 +480,32 @@ slp_status pin_range(L* h, const void* p, size_t bytes, const char* what) {
   if (e == cudaSuccess && attr.type == cudaMemoryTypeDevice)
     return fail(SLP_ERR_INVALID_ARG, "%s is a device pointer; host weights are expected", what);
   cudaGetLastError();
-  {
-    std::lock_guard<std::mutex> lock(g_reg_mutex);
-    auto it = g_registered.find(const_cast<void*>(p));
-    if (it != g_registered.end()) {  // registered by another handle of this process: share it
-      ++it->second;
-      h->registered.push_back(const_cast<void*>(p));
-      return SLP_OK;
-    }
+  // One lock over lookup, registration and insertion: two threads creating handles over the same host copy must not
+  // both see "not registered yet", or one of them would hold the range without a reference and lose it at the
+  // other's destroy.
+  std::lock_guard<std::mutex> lock(g_reg_mutex);
+  auto it = g_registered.find(const_cast<void*>(p));
+  if (it != g_registered.end() && bytes <= it->second.bytes) {  // registered by another handle of this process: share it
+    ++it->second.refs;
+    h->registered.push_back(const_cast<void*>(p));
+    return SLP_OK;
   }
+  // (a range that starts at a registered pointer but is LONGER than what was registered, e.g. the full expert stack
+  // after a shard of it, is not covered by that entry: it goes through the checks below like any other range)
   if (range_is_pinned(p, bytes)) return SLP_OK;
   if (h->cfg.require_pinned) return fail(SLP_ERR_NOT_PINNED, "%s is pageable host memory and require_pinned is set", what);
   e = cudaHostRegister(const_cast<void*>(p), bytes, cudaHostRegisterDefault);
   if (e == cudaErrorHostMemoryAlreadyRegistered) {
-    // part of the range (a page shared with a neighbouring tensor) was registered before: accept only if
-    // the whole range is page-locked now, otherwise the copies would silently fall back to staged transfers
+    // part of the range (a page shared with a neighbouring tensor, or a shorter range another handle registered) was
+    // registered before: accept only if the whole range is page-locked now, otherwise the copies would silently fall
+    // back to staged transfers
     cudaGetLastError();
     if (range_is_pinned(p, bytes)) return SLP_OK;
     return fail(SLP_ERR_NOT_PINNED, "%s overlaps an already registered range but is not page-locked end to end; "
                                     "register the enclosing allocation once or pass pinned memory", what);
   }
   if (e != cudaSuccess) return fail(SLP_ERR_NOT_PINNED, "cudaHostRegister(%s, %zu bytes) failed: %s", what, bytes, cudaGetErrorString(e));
-  {
-    std::lock_guard<std::mutex> lock(g_reg_mutex);
-    g_registered[const_cast<void*>(p)] = 1;
-  }
+  g_registered[const_cast<void*>(p)] = Registered{1, bytes};
   h->registered.push_back(const_cast<void*>(p));
   return SLP_OK;
 }

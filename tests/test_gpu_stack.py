@@ -200,3 +200,46 @@ def test_two_handles_share_one_pageable_host_copy():
     with pytest.raises(SlpError) as ei:
         SlpMoeLayer(cfg, W, device=0, require_pinned=True)
     assert ei.value.status == -5
+
+
+def test_longer_range_at_a_registered_pointer_is_not_taken_for_pinned():
+    """A shard handle page-locks experts [0, E/2) of a pageable stack; a second handle over all E experts starts at
+    the SAME host pointer but needs twice the bytes.  It must not ride on the shorter registration: either create
+    refuses (NOT_PINNED: the range is not page-locked end to end) or the whole range is page-locked afterwards."""
+    cfg, _, hidden, _ = problem("mini_dsv3")
+    W = inputs.make_weights(cfg, device="cpu", pin=False)
+    cudart = ctypes.CDLL("libcudart.so.12")
+    g = W["gate_q"]
+    tail_ptr, tail_bytes = g[cfg.E - 1].data_ptr(), g[cfg.E - 1].numel()
+
+    def tail_is_registered():
+        rc = cudart.cudaHostRegister(ctypes.c_void_p(tail_ptr), ctypes.c_size_t(tail_bytes), 0)
+        if rc == 0:
+            cudart.cudaHostUnregister(ctypes.c_void_p(tail_ptr))
+            return False
+        cudart.cudaGetLastError()
+        return True
+
+    a = SlpMoeLayer(cfg, W, device=0, expert_range=(0, cfg.E // 2))
+    try:
+        assert not tail_is_registered()
+        try:
+            b = SlpMoeLayer(cfg, W, device=0)
+        except SlpError as e:
+            assert e.status == -5 and "page-locked end to end" in str(e)
+        else:
+            try:
+                assert tail_is_registered(), "create accepted a range whose tail is pageable"
+            finally:
+                b.close()
+    finally:
+        a.close()
+    assert not tail_is_registered()
+    full = SlpMoeLayer(cfg, W, device=0)     # with the shard gone the full stack registers normally
+    try:
+        assert tail_is_registered()
+        out = full.prefill(hidden.cuda())
+        torch.cuda.synchronize()
+        assert torch.isfinite(out.float()).all()
+    finally:
+        full.close()
