@@ -34,6 +34,8 @@
 extern "C" {
 #endif
 
+#define SLP_MOE_ABI_VERSION 3u /* layout and meaning of the structs below; checked by create and query_plan */
+
 typedef struct slp_moe_layer slp_moe_layer; /* opaque handle */
 
 typedef enum {
@@ -83,6 +85,10 @@ typedef struct {
                                  token over all E experts, but copies, stores and runs only its own experts; the host
                                  pointers of the other experts may be NULL.  It is driven through
                                  slp_moe_prefill_partial; staging_slots counts this handle's experts. */
+  uint32_t abi_version;       /* = SLP_MOE_ABI_VERSION of the header the caller was built with.  Fields of this struct
+                                 have changed meaning in place before (gemm_impl / router_impl became expert_begin /
+                                 expert_end at the same size); from ABI 3 on any such change bumps this number, and a
+                                 caller built against an older header is refused (by struct_size: the field is new). */
 } slp_moe_cfg;
 
 /* Host weight pointers.  Borrowed for the lifetime of the handle; the host copy stays
@@ -315,7 +321,7 @@ slp_status slp_moe_permute_static(int32_t device, const int32_t* idx_dev, int32_
  * roundup128(T) + roundup128(T * top_k + 127 * n_experts); -1 for a negative argument. */
 int64_t slp_moe_permute_static_rows(int32_t T, int32_t top_k, int32_t n_experts);
 
-/* Library version string. */
+/* Library version string, "slpmoe <release> (sm_100a; abi <SLP_MOE_ABI_VERSION>)". */
 const char* slp_version(void);
 
 #ifdef __cplusplus

@@ -22,6 +22,7 @@ EXPORTED_SYMBOLS = [
 ]
 
 SLP_STREAMED, SLP_RESIDENT = 0, 1
+ABI_VERSION = 3   # SLP_MOE_ABI_VERSION of include/slp_moe.h
 SCORING = {"sigmoid_bias": 0, "softmax": 1}
 BUF = dict(counts=0, row_start=1, pos=2, row_token=3, hq=4, hs=5, y=6, logits=7, ys=8)
 
@@ -40,7 +41,8 @@ class _Cfg(C.Structure):
                 ("scoring", C.c_int32), ("norm_topk", C.c_int32), ("routed_scale", C.c_float),
                 ("max_tokens", C.c_int32), ("staging_slots", C.c_int32),
                 ("experts_per_launch", C.c_int32), ("skip_empty_experts", C.c_int32),
-                ("require_pinned", C.c_int32), ("expert_begin", C.c_int32), ("expert_end", C.c_int32)]
+                ("require_pinned", C.c_int32), ("expert_begin", C.c_int32), ("expert_end", C.c_int32),
+                ("abi_version", C.c_uint32)]
 
 
 class _HostWeights(C.Structure):
@@ -153,7 +155,8 @@ def _make_cfg(cfg, *, max_tokens=None, device=0, staging_slots=0, experts_per_la
                 routed_scale=cfg.routed_scale, max_tokens=max_tokens or cfg.T,
                 staging_slots=staging_slots, experts_per_launch=experts_per_launch,
                 skip_empty_experts=int(skip_empty_experts), require_pinned=int(require_pinned),
-                expert_begin=expert_range[0] if expert_range else 0, expert_end=expert_range[1] if expert_range else 0)
+                expert_begin=expert_range[0] if expert_range else 0, expert_end=expert_range[1] if expert_range else 0,
+                abi_version=ABI_VERSION)
 
 
 def query_plan(cfg, **kw):

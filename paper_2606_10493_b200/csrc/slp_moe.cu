@@ -933,7 +933,7 @@ slp_status prefetch_layer(L* h, int l) {
 extern "C" {
 
 const char* slp_last_error(void) { return g_last_error.c_str(); }
-const char* slp_version(void) { return "slpmoe 0.1 (sm_100a)"; }
+const char* slp_version(void) { return "slpmoe 0.3 (sm_100a; abi 3)"; }
 
 
 slp_status slp_moe_layer_create(const slp_moe_cfg* cfg, const slp_moe_host_weights* w, slp_moe_layer** out) {
@@ -944,7 +944,11 @@ slp_status slp_moe_stack_create(const slp_moe_cfg* cfg, int32_t n_layers, const 
   if (!cfg || !w_all || !out) return fail(SLP_ERR_INVALID_ARG, "NULL argument");
   if (n_layers < 1 || n_layers > 4096) return fail(SLP_ERR_INVALID_ARG, "n_layers %d outside 1..4096", n_layers);
   const slp_moe_host_weights* w = w_all;
-  if (cfg->struct_size != sizeof(slp_moe_cfg)) return fail(SLP_ERR_INVALID_ARG, "cfg.struct_size %u != %zu", cfg->struct_size, sizeof(slp_moe_cfg));
+  if (cfg->struct_size != sizeof(slp_moe_cfg))
+    return fail(SLP_ERR_INVALID_ARG, "cfg.struct_size %u != %zu: the caller was built against another slp_moe.h (this library: ABI %u)",
+                cfg->struct_size, sizeof(slp_moe_cfg), SLP_MOE_ABI_VERSION);
+  if (cfg->abi_version != SLP_MOE_ABI_VERSION)
+    return fail(SLP_ERR_INVALID_ARG, "cfg.abi_version %u, this library implements ABI %u", cfg->abi_version, SLP_MOE_ABI_VERSION);
   *out = nullptr;
   const int H = cfg->hidden, E = cfg->n_experts, k = cfg->top_k, I = cfg->moe_intermediate;
   int n_stage = 0, epl = 0;
@@ -1150,7 +1154,11 @@ slp_status slp_moe_stack_create(const slp_moe_cfg* cfg, int32_t n_layers, const 
 
 slp_status slp_moe_query_plan(const slp_moe_cfg* cfg, slp_moe_plan* plan) {
   if (!cfg || !plan) return fail(SLP_ERR_INVALID_ARG, "NULL argument");
-  if (cfg->struct_size != sizeof(slp_moe_cfg)) return fail(SLP_ERR_INVALID_ARG, "cfg.struct_size %u != %zu", cfg->struct_size, sizeof(slp_moe_cfg));
+  if (cfg->struct_size != sizeof(slp_moe_cfg))
+    return fail(SLP_ERR_INVALID_ARG, "cfg.struct_size %u != %zu: the caller was built against another slp_moe.h (this library: ABI %u)",
+                cfg->struct_size, sizeof(slp_moe_cfg), SLP_MOE_ABI_VERSION);
+  if (cfg->abi_version != SLP_MOE_ABI_VERSION)
+    return fail(SLP_ERR_INVALID_ARG, "cfg.abi_version %u, this library implements ABI %u", cfg->abi_version, SLP_MOE_ABI_VERSION);
   if (plan->struct_size != sizeof(slp_moe_plan)) return fail(SLP_ERR_INVALID_ARG, "plan.struct_size mismatch");
   int n_stage = 0, epl = 0;
   slp_status st = validate_cfg(cfg, &n_stage, &epl);

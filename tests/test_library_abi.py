@@ -31,8 +31,11 @@ def test_exports_every_declared_symbol(built):
 
 
 def test_struct_sizes_match_header(built):
-    # 20 four-byte fields / 14 pointers / see header
-    assert ctypes.sizeof(binding._Cfg) == 20 * 4
+    # 21 four-byte fields / 14 pointers / see header
+    assert ctypes.sizeof(binding._Cfg) == 21 * 4
+    header = open(os.path.join(ROOT, "include", "slp_moe.h")).read()
+    assert int(re.search(r"#define SLP_MOE_ABI_VERSION (\d+)u", header).group(1)) == binding.ABI_VERSION
+    assert f"abi {binding.ABI_VERSION})".encode() in built.slp_version()
     assert ctypes.sizeof(binding._HostWeights) == 14 * 8
     assert ctypes.sizeof(binding.Stats) == 120  # ... + experts_from_prefetch, experts_prefetched, layer, (pad), bytes_prefetched, ms_gateup_shared, ms_down_shared
 
@@ -45,6 +48,15 @@ def test_invalid_arguments_are_reported(built):
     hw = binding._HostWeights()
     assert built.slp_moe_layer_create(ctypes.byref(cfg), ctypes.byref(hw), ctypes.byref(out)) == -1
     assert b"struct_size" in built.slp_last_error()
+    # a caller built against the previous header (20 fields, gemm_impl / router_impl where the expert range is now)
+    stale = binding._Cfg(struct_size=80)
+    assert built.slp_moe_layer_create(ctypes.byref(stale), ctypes.byref(hw), ctypes.byref(out)) == -1
+    assert b"another slp_moe.h" in built.slp_last_error()
+    wrong = binding._make_cfg(inputs.CONFIGS[0])
+    wrong.abi_version = 2
+    plan = binding.Plan(struct_size=ctypes.sizeof(binding.Plan))
+    assert built.slp_moe_query_plan(ctypes.byref(wrong), ctypes.byref(plan)) == -1
+    assert b"abi_version 2" in built.slp_last_error()
     assert built.slp_moe_prefill(None, None, 1, None, None) == -1
     assert built.slp_moe_layer_destroy(None) == 0
 
