@@ -199,7 +199,8 @@ slp_status slp_moe_stack_create(const slp_moe_cfg* cfg, int32_t n_layers, const 
 slp_status slp_moe_stack_prefill(slp_moe_layer* h, int32_t layer, const void* hidden_bf16, int32_t T, void* out_bf16, void* cuda_stream);
 
 /* Explicit loader run-ahead: enqueue the copies of `layer` now (as many launch groups as the ring has slots that
- * hold no unconsumed prefetch).  Returns immediately; a later slp_moe_stack_prefill(layer) consumes them. */
+ * hold no unconsumed prefetch of that same layer; an unconsumed prefetch of another layer is overwritten).  Returns
+ * immediately; a later slp_moe_stack_prefill(layer) consumes them. */
 slp_status slp_moe_stack_prefetch(slp_moe_layer* h, int32_t layer);
 
 /* Validates cfg exactly as create does and fills *plan; needs no GPU and allocates nothing.
@@ -244,6 +245,12 @@ slp_status slp_moe_prefill(slp_moe_layer* h, const void* hidden_bf16, int32_t T,
  *  (then the partial sum is the whole layer in fp32).  Ordering, copy stream and error rules as slp_moe_prefill. */
 slp_status slp_moe_prefill_partial(slp_moe_layer* h, const void* hidden_bf16, int32_t T, float* partial_f32,
                                    int32_t shared_token_begin, int32_t shared_token_end, void* cuda_stream);
+
+/* slp_moe_prefill_partial on layer `layer` of a stack (slp_moe_prefill_partial itself addresses layer 0), with the same
+ * run-ahead of layer (layer + 1) % n_layers as slp_moe_stack_prefill: SmallEP over a multi-layer, expert-sharded stack.
+ * INVALID_ARG for a layer outside the stack. */
+slp_status slp_moe_stack_prefill_partial(slp_moe_layer* h, int32_t layer, const void* hidden_bf16, int32_t T, float* partial_f32,
+                                         int32_t shared_token_begin, int32_t shared_token_end, void* cuda_stream);
 
 /* out_bf16[i] = bf16_rne(sum_f32[i]) for n_elems elements (multiple of 4) on `device`: the single output rounding
  * of the SmallEP path, applied to the reduce-scattered sum.  Asynchronous on cuda_stream. */

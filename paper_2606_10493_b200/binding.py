@@ -18,7 +18,7 @@ EXPORTED_SYMBOLS = [
     "slp_measure_h2d", "slp_version", "slp_moe_query_plan", "slp_moe_debug_buffer_range",
     "slp_moe_prefill_partial", "slp_moe_finalize_partial",
     "slp_moe_stack_create", "slp_moe_stack_prefill", "slp_moe_stack_prefetch",
-    "slp_moe_permute_static", "slp_moe_permute_static_rows",
+    "slp_moe_permute_static", "slp_moe_permute_static_rows", "slp_moe_stack_prefill_partial",
 ]
 
 SLP_STREAMED, SLP_RESIDENT = 0, 1
@@ -93,6 +93,7 @@ def lib():
         L.slp_moe_set_residency.argtypes = [C.c_void_p, C.c_int]
         L.slp_moe_prefill.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
         L.slp_moe_prefill_partial.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p]
+        L.slp_moe_stack_prefill_partial.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p]
         L.slp_moe_finalize_partial.argtypes = [C.c_int32, C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p]
         L.slp_moe_prefill_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
         L.slp_moe_layer_destroy.argtypes = [C.c_void_p]
@@ -271,17 +272,18 @@ class SlpMoeLayer:
         """slp_moe_stack_prefetch: let the loader run ahead with `layer`'s expert copies."""
         _check(lib().slp_moe_stack_prefetch(self._h, layer))
 
-    def prefill_partial(self, hidden_all, partial=None, shared_tokens=(0, 0), stream=None):
+    def prefill_partial(self, hidden_all, partial=None, shared_tokens=(0, 0), stream=None, layer=0):
         """SmallEP: hidden_all = the all-gathered CUDA bf16 [T, H] hidden states; returns the fp32 [T, H] partial
-        weighted sum over this handle's experts (+ the shared expert for tokens in `shared_tokens`)."""
+        weighted sum over this handle's experts (+ the shared expert for tokens in `shared_tokens`).  `layer`: which
+        layer of a multi-layer stack (slp_moe_stack_prefill_partial)."""
         import torch
         assert hidden_all.is_cuda and hidden_all.dtype == torch.bfloat16 and hidden_all.is_contiguous()
         if partial is None:
             partial = torch.empty(hidden_all.shape, dtype=torch.float32, device=hidden_all.device)
         assert partial.dtype == torch.float32 and partial.is_contiguous() and partial.shape == hidden_all.shape
         s = torch.cuda.current_stream(hidden_all.device) if stream is None else stream
-        _check(lib().slp_moe_prefill_partial(self._h, hidden_all.data_ptr(), hidden_all.shape[0], partial.data_ptr(),
-                                             int(shared_tokens[0]), int(shared_tokens[1]), s.cuda_stream))
+        _check(lib().slp_moe_stack_prefill_partial(self._h, layer, hidden_all.data_ptr(), hidden_all.shape[0], partial.data_ptr(),
+                                                   int(shared_tokens[0]), int(shared_tokens[1]), s.cuda_stream))
         return partial
 
     def prefill_host(self, hidden_host, out_host):

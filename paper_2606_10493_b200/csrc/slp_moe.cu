@@ -906,8 +906,9 @@ slp_status prefill_impl(L* h, const void* hidden, int T, void* out, cudaStream_t
   return SLP_OK;
 }
 
-// Loader run-ahead: enqueue the copies of layer l's launch groups into the ring (one pass over the ring at most),
-// stopping at the first slot that still holds a prefetch nobody consumed.  Each copy waits for the OFF event of the
+// Loader run-ahead: enqueue the copies of layer l's launch groups into the ring (one pass over the ring at most);
+// slots that already hold an unconsumed prefetch of the same group are kept, unconsumed prefetches of anything else are
+// overwritten.  Each copy waits for the OFF event of the
 // launch that last used its slot.  Leaves layer l selected.
 slp_status prefetch_layer(L* h, int l) {
   if (h->residency != SLP_STREAMED) return SLP_OK;
@@ -916,7 +917,13 @@ slp_status prefetch_layer(L* h, int l) {
   int grp = 0;
   for (int e0 = h->e0; e0 < h->e1 && grp < n_ring; e0 += epl, ++grp) {
     const int e1 = std::min(h->e1, e0 + epl), r = grp % n_ring;
-    if (h->occ_prefetched[r]) break;
+    if (h->occ_prefetched[r]) {
+      if (h->occ_layer[r] == l && h->occ_e0[r] == e0) continue;  // this very group is already loaded (or loading)
+      // A prefetch for another layer or group that no call consumed (layers called out of order; its group turned out
+      // empty under skip_empty_experts): it would otherwise sit there for ever and stop every later run-ahead at this
+      // slot.  Overwrite it: the copy stream is in order, so the new copy follows the stale one, and the wait below
+      // covers the last launch that read the slot.
+    }
     if (h->free_recorded[r]) CU_TRY(cudaStreamWaitEvent(h->copy_stream, h->ev_free[r], 0));
     slp_status st = copy_experts(h, e0, e1, nullptr);
     if (st != SLP_OK) return st;
@@ -1277,7 +1284,13 @@ slp_status slp_moe_stack_prefill(slp_moe_layer* h, int32_t layer, const void* hi
 
 slp_status slp_moe_prefill_partial(slp_moe_layer* h, const void* hidden_bf16, int32_t T, float* partial_f32, int32_t sh_t0, int32_t sh_t1,
                                    void* cuda_stream) {
+  return slp_moe_stack_prefill_partial(h, 0, hidden_bf16, T, partial_f32, sh_t0, sh_t1, cuda_stream);
+}
+
+slp_status slp_moe_stack_prefill_partial(slp_moe_layer* h, int32_t layer, const void* hidden_bf16, int32_t T, float* partial_f32,
+                                         int32_t sh_t0, int32_t sh_t1, void* cuda_stream) {
   if (!h) return fail(SLP_ERR_INVALID_ARG, "NULL handle");
+  if (layer < 0 || layer >= static_cast<int>(h->layers.size())) return fail(SLP_ERR_INVALID_ARG, "layer %d outside 0..%zu", layer, h->layers.size() - 1);
   if (T < 0 || T > h->Tm) return fail(SLP_ERR_INVALID_ARG, "T = %d outside 0..max_tokens (%d)", T, h->Tm);
   if (T == 0) return SLP_OK;
   if (!hidden_bf16 || !partial_f32) return fail(SLP_ERR_INVALID_ARG, "NULL hidden/partial");
@@ -1297,7 +1310,7 @@ slp_status slp_moe_prefill_partial(slp_moe_layer* h, const void* hidden_bf16, in
       return fail(SLP_ERR_CUDA, "cudaEventQuery failed: %s", cudaGetErrorString(q));
     }
   }
-  return prefill_impl(h, hidden_bf16, T, partial_f32, s, true, sh_t0, sh_t1);
+  return prefill_impl(h, hidden_bf16, T, partial_f32, s, true, sh_t0, sh_t1, layer);
 }
 
 slp_status slp_moe_finalize_partial(int32_t device, const float* sum_f32, size_t n_elems, void* out_bf16, void* cuda_stream) {

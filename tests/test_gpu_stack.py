@@ -243,3 +243,64 @@ def test_longer_range_at_a_registered_pointer_is_not_taken_for_pinned():
         assert torch.isfinite(out.float()).all()
     finally:
         full.close()
+
+
+def test_a_later_prefetch_replaces_an_unconsumed_one(layers):
+    """Run-ahead for layer 2 that nobody consumes must not block the ring: a following prefetch of layer 1 overwrites
+    it, and the call on layer 1 then finds all its experts loaded ahead (and computes the right thing)."""
+    cfgs, Ws, hidden, singles = layers
+    cfg = cfgs[0]
+    stack = SlpMoeLayer(cfg, Ws, device=0)
+    try:
+        stack.prefetch(2)
+        stack.prefetch(1)
+        stack.prefetch(1)                                  # same groups again: kept, not copied twice
+        out = stack.prefill(hidden, layer=1).clone()
+        torch.cuda.synchronize()
+        st = stack.stats()
+        assert st["experts_from_prefetch"] == cfg.E and st["experts_copied"] == 0, st
+        assert torch.equal(out.view(torch.int16), singles[1].view(torch.int16))
+        out0 = stack.prefill(hidden, layer=0).clone()      # out of order: layer 2 was prefetched behind layer 1, layer 0 is asked for
+        torch.cuda.synchronize()
+        assert stack.stats()["experts_copied"] == cfg.E
+        assert torch.equal(out0.view(torch.int16), singles[0].view(torch.int16))
+    finally:
+        stack.close()
+
+
+def test_partial_sums_address_the_layers_of_a_stack(layers):
+    """slp_moe_stack_prefill_partial: the fp32 partial path on layer l of a stack.  Unsharded, rounded once, it is
+    slp_moe_prefill of that layer bit for bit; over two expert-sharded stacks the partial sums add up to it (to the
+    bf16 step the different association of the fp32 additions allows)."""
+    from paper_2606_10493_b200 import finalize_partial, smallep
+    cfgs, Ws, hidden, singles = layers
+    cfg = cfgs[0]
+    stack = SlpMoeLayer(cfg, Ws, device=0)
+    try:
+        for l in (2, 0, 1):
+            p = stack.prefill_partial(hidden, shared_tokens=(0, cfg.T), layer=l)
+            torch.cuda.synchronize()
+            assert stack.stats()["layer"] == l
+            assert torch.equal(finalize_partial(p).view(torch.int16), singles[l].view(torch.int16)), l
+        with pytest.raises(SlpError) as ei:
+            stack.prefill_partial(hidden, shared_tokens=(0, cfg.T), layer=N_LAYERS)
+        assert ei.value.status == -1
+    finally:
+        stack.close()
+    G = 2
+    shards = [SlpMoeLayer(cfg, Ws, device=0, expert_range=smallep.expert_range(cfg.E, r, G)) for r in range(G)]
+    try:
+        for l in range(N_LAYERS):
+            total = None
+            for r, sh in enumerate(shards):
+                t0, t1 = r * cfg.T // G, (r + 1) * cfg.T // G
+                p = sh.prefill_partial(hidden, shared_tokens=(t0, t1), layer=l)
+                torch.cuda.synchronize()
+                total = p.clone() if total is None else total + p
+            out = finalize_partial(total)
+            a, b = out.float(), singles[l].float()
+            rms = float(b.pow(2).mean().sqrt())
+            assert bool(((a - b).abs() <= 2.0 ** -7 * b.abs() + 1e-3 * rms).all()), l
+    finally:
+        for sh in shards:
+            sh.close()
