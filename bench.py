@@ -263,7 +263,7 @@ def main(argv=None):
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip the resident / 32K / soak / fp8-peak extras of the default run")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
-    ap.add_argument("--triage", default=None, help="SLP_TRIAGE value for A/B runs (e.g. gemm=pair); not a product option")
+    ap.add_argument("--triage", default=None, help="triage spec (slp_moe_debug_set_triage) for A/B runs (e.g. gemm=pair); not a product option")
     ap.add_argument("--staging-slots", type=int, default=0)
     ap.add_argument("--experts-per-launch", type=int, default=0)
     args = ap.parse_args(argv)

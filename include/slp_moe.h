@@ -277,6 +277,13 @@ slp_status slp_moe_debug_buffer(slp_moe_layer* h, int32_t which, void* host_dst,
 slp_status slp_moe_debug_buffer_range(slp_moe_layer* h, int32_t which, size_t offset, size_t bytes, void* host_dst);
 slp_status slp_moe_get_stats(slp_moe_layer* h, slp_moe_stats* stats);
 
+/* Bring-up / bisection only, not a product option: the NEXT slp_moe_layer_create / slp_moe_stack_create on the calling
+ * thread builds its handle with the kernel variants or the workspace canary bands `spec` names (comma-separated:
+ * "gemm=simt", "gemm=static", "gemm=pair", "router=fp32", "guards", "guards=selftest"), then the setting is
+ * gone.  NULL or "" = the product path (and cancels a pending setting).  Thread-local: creates on other threads are
+ * not affected, and the library reads no environment variable.  INVALID_ARG for an unknown token. */
+slp_status slp_moe_debug_set_triage(const char* spec);
+
 /* Measures pinned host -> device bandwidth on `device` with back-to-back cudaMemcpyAsync of
  * `chunk_bytes` each (total `total_bytes`, best of `repeats`); writes GB/s (1e9) to *gbs.
  * This is the denominator of the streamed-mode roofline. */

@@ -19,6 +19,7 @@ EXPORTED_SYMBOLS = [
     "slp_moe_prefill_partial", "slp_moe_finalize_partial",
     "slp_moe_stack_create", "slp_moe_stack_prefill", "slp_moe_stack_prefetch",
     "slp_moe_permute_static", "slp_moe_permute_static_rows", "slp_moe_stack_prefill_partial",
+    "slp_moe_debug_set_triage",
 ]
 
 SLP_STREAMED, SLP_RESIDENT = 0, 1
@@ -101,6 +102,7 @@ def lib():
         L.slp_moe_debug_quant_hidden.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.slp_moe_debug_buffer.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_size_t, C.POINTER(C.c_size_t)]
         L.slp_moe_debug_buffer_range.argtypes = [C.c_void_p, C.c_int32, C.c_size_t, C.c_size_t, C.c_void_p]
+        L.slp_moe_debug_set_triage.argtypes = [C.c_char_p]
         L.slp_moe_get_stats.argtypes = [C.c_void_p, C.POINTER(Stats)]
         L.slp_measure_h2d.argtypes = [C.c_int32, C.c_size_t, C.c_size_t, C.c_int32, C.POINTER(C.c_double)]
         L.slp_moe_permute_static.argtypes = [C.c_int32, C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p,
@@ -210,9 +212,9 @@ class SlpMoeLayer:
     def __init__(self, cfg, weights, *, max_tokens=None, device=0, staging_slots=0,
                  experts_per_launch=0, skip_empty_experts=False, require_pinned=False, triage=None, expert_range=None):
         """`expert_range` = (e0, e1): the handle owns routed experts [e0, e1) only (SmallEP); `weights` may then
-        hold just that shard (inputs.make_weights(..., shard=(e0, e1))).  `triage`: value for the library's
-        SLP_TRIAGE environment switch during create (e.g. "gemm=simt", "gemm=pair,router=fp32"); bring-up /
-        bisection only, not part of the ABI."""
+        hold just that shard (inputs.make_weights(..., shard=(e0, e1))).  `triage`: kernel-variant / canary-band
+        selection for this one create (slp_moe_debug_set_triage, e.g. "gemm=simt", "gemm=pair,router=fp32");
+        bring-up / bisection only."""
         self._h = C.c_void_p()
         self.cfg = cfg
         self.weights = weights
@@ -240,17 +242,13 @@ class SlpMoeLayer:
                 setattr(hw, name, p(w[name]))
             for k, arr in arrays.items():
                 setattr(hw, k, C.cast(arr, C.POINTER(C.c_void_p)))
-        saved = os.environ.get("SLP_TRIAGE")
         if triage is not None:
-            os.environ["SLP_TRIAGE"] = triage
+            _check(lib().slp_moe_debug_set_triage(triage.encode()))   # thread-local, consumed by the create below
         try:
             _check(lib().slp_moe_stack_create(C.byref(c), self.n_layers, hws, C.byref(self._h)))
         finally:
             if triage is not None:
-                if saved is None:
-                    os.environ.pop("SLP_TRIAGE", None)
-                else:
-                    os.environ["SLP_TRIAGE"] = saved
+                lib().slp_moe_debug_set_triage(None)                   # in case create failed before taking it
 
     # -- the C-ABI calls ------------------------------------------------------------------
     def set_residency(self, mode):
@@ -332,7 +330,7 @@ class SlpMoeLayer:
     def close(self):
         if self._h:
             h, self._h = self._h, C.c_void_p()
-            _check(lib().slp_moe_layer_destroy(h))   # non-zero only under SLP_TRIAGE=guards (a canary band was written)
+            _check(lib().slp_moe_layer_destroy(h))   # non-zero only under triage "guards" (a canary band was written)
 
     def __del__(self):
         try:

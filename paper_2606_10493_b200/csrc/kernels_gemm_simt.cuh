@@ -1,4 +1,4 @@
-// kernels_gemm_simt.cuh — plain CUDA-core grouped FP8 GEMM (SLP_TRIAGE gemm=simt).
+// kernels_gemm_simt.cuh — plain CUDA-core grouped FP8 GEMM (triage "gemm=simt").
 // Bring-up / triage scaffolding for the tcgen05 kernel in kernels_gemm_tc.cuh: same inputs, same
 // outputs, same block-scale promotion structure (one fp32 partial per 128-deep K block, scaled by
 // xs[row, kb] * ws[nb, kb] and added into an fp32 accumulator), but no tensor cores, no TMA.

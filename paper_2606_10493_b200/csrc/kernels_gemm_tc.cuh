@@ -3,7 +3,7 @@
 // One persistent CTA per SM works through the (128-row tile, N tile) work items of the experts of the
 // launch (one 16-byte record per tile, written by permute_scan_kernel); an otherwise idle warp takes the
 // items from a global counter, so all CTAs stay within ~gridDim consecutive items and share operands
-// through L2 (SLP_TRIAGE gemm=static: static round-robin instead).  Per 128-deep K block the tensor core
+// through L2 (triage "gemm=static": static round-robin instead).  Per 128-deep K block the tensor core
 // writes a fresh 128 x 256 fp32 partial into TMEM, as two independent 128-column halves (four half-buffers
 // in flight); the promotion warps pull it out with tcgen05.ld and add it into fp32 register accumulators
 // with one FMA per element (issued as FFMA2 pairs), scaled by  xs[row, kb] * ws[n-block, kb]
@@ -24,7 +24,7 @@
 //               of half w / 4; 128 fp32 accumulators per thread; a half-buffer is handed back as soon as
 //               the last tcgen05.ld has landed, before the last FMAs
 //
-// kPair (SLP_TRIAGE gemm=pair): a cluster of two CTAs issues cta_group::2 MMAs with M = 256 (two
+// kPair (triage "gemm=pair"): a cluster of two CTAs issues cta_group::2 MMAs with M = 256 (two
 //   128-row tiles of the same expert) x N = 128 per column half; each CTA stages its own A tile and half of
 //   the B tile (CTA 0 the gate rows / CTA 1 the up rows of a gate/up tile; 64 rows of each column half of a
 //   down tile); TMA loads of both CTAs complete on the leader's mbarrier, commits are multicast to both CTAs,
@@ -202,7 +202,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
   };
 
   // Tile that follows this CTA's i-th one (e < 0: none).  Static order: item w + gridDim, record read from global
-  // memory.  kDyn (one-CTA kernel, the default; SLP_TRIAGE gemm=static selects the static order): items come from a
+  // memory.  kDyn (one-CTA kernel, the default; triage "gemm=static" selects the static order): items come from a
   // global counter, so all CTAs stay inside a window of ~gridDim consecutive items and the B tiles they share stay in
   // L2 (profiles/r1_sched_ab.md).  An otherwise idle warp takes the item AND reads its record, and publishes the
   // record through a four-deep ring in shared memory: the roles pay one barrier wait and one 16-byte shared load per

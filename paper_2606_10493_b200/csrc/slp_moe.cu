@@ -109,9 +109,10 @@ constexpr int kTailExperts = 8;  // experts per launch inside the last launch gr
 
 inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
 
-// Triage switches, read once per create from the environment variable SLP_TRIAGE (comma-separated tokens);
-// not part of the ABI.  They select bring-up / A-B variants of two kernels so a wrong result can be
-// bisected on a GPU box without rebuilding:
+// Triage switches (not a product option): bring-up / A-B variants of two kernels, so a wrong result can be bisected
+// on a GPU box without rebuilding.  They are handed over per thread through slp_moe_debug_set_triage() and consumed by
+// the next create on that thread; the library reads no environment variable, so nothing in a process's environment can
+// change which kernels a handle runs.  Comma-separated tokens:
 //   gemm=simt    plain CUDA-core grouped GEMM (kernels_gemm_simt.cuh) instead of the tcgen05 kernels
 //   gemm=static  one-CTA tcgen05 kernel with the static round-robin tile order
 //   gemm=pair    the cta_group::2 variant of the tcgen05 kernel
@@ -125,17 +126,31 @@ struct Triage {
   int router_fp32 = 0;
   int guards = 0;
 };
+thread_local Triage g_triage_next;  // what the next create on this thread takes (default: the product path)
+
+// Parses a triage spec; false (and *bad = the offending token) on an unknown token.
+bool parse_triage(const std::string& v, Triage* t, std::string* bad) {
+  size_t pos = 0;
+  while (pos <= v.size()) {
+    size_t end = v.find(',', pos);
+    if (end == std::string::npos) end = v.size();
+    const std::string tok = v.substr(pos, end - pos);
+    if (tok.empty()) {}
+    else if (tok == "gemm=simt") t->gemm = kGemmSimt;
+    else if (tok == "gemm=static") t->gemm = kGemmStatic;
+    else if (tok == "gemm=pair") t->gemm = kGemmPair;
+    else if (tok == "router=fp32") t->router_fp32 = 1;
+    else if (tok == "guards") t->guards = std::max(t->guards, 1);
+    else if (tok == "guards=selftest") t->guards = 2;  // create damages one band on purpose (negative control)
+    else { *bad = tok; return false; }
+    pos = end + 1;
+  }
+  return true;
+}
+
 inline Triage read_triage() {
-  Triage t;
-  const char* env = std::getenv("SLP_TRIAGE");
-  if (!env) return t;
-  const std::string v(env);
-  if (v.find("gemm=simt") != std::string::npos) t.gemm = kGemmSimt;
-  else if (v.find("gemm=static") != std::string::npos) t.gemm = kGemmStatic;
-  else if (v.find("gemm=pair") != std::string::npos) t.gemm = kGemmPair;
-  if (v.find("router=fp32") != std::string::npos) t.router_fp32 = 1;
-  if (v.find("guards") != std::string::npos) t.guards = 1;
-  if (v.find("guards=selftest") != std::string::npos) t.guards = 2;  // create damages one band on purpose (negative control)
+  const Triage t = g_triage_next;
+  g_triage_next = Triage{};
   return t;
 }
 
@@ -246,7 +261,7 @@ struct slp_moe_layer {
   std::vector<cudaEvent_t> ev_k;  // 3 events per expert launch pair: before gate/up, between, after down
   std::vector<cudaEvent_t> ev_tail;  // ON events of the pieces of a call's last launch group
   struct Guarded { void* base; void* user; size_t bytes; const char* name; };
-  std::vector<Guarded> guarded;      // SLP_TRIAGE=guards: workspace allocations with canary bands
+  std::vector<Guarded> guarded;      // triage "guards": workspace allocations with canary bands
   int ev_k_used = 0;
   int ev_k_shared = -1;  // first event of the shared expert's own launch pair in ev_k (-1: it shares a launch with routed experts)
 };
@@ -255,7 +270,7 @@ namespace {
 
 using L = slp_moe_layer;
 
-// Workspace allocation.  With SLP_TRIAGE=guards every buffer sits between two 4 KB canary bands (0xA5) that
+// Workspace allocation.  With triage "guards" every buffer sits between two 4 KB canary bands (0xA5) that
 // check_guards() reads back: a kernel that writes outside a buffer (the usual way a tile-bookkeeping bug shows) is
 // caught without compute-sanitizer, which is closed on the GPU pool.
 constexpr size_t kGuardBytes = 4096;
@@ -940,6 +955,14 @@ slp_status prefetch_layer(L* h, int l) {
 extern "C" {
 
 const char* slp_last_error(void) { return g_last_error.c_str(); }
+
+slp_status slp_moe_debug_set_triage(const char* spec) {
+  Triage t;
+  std::string bad;
+  if (spec && !parse_triage(spec, &t, &bad)) return fail(SLP_ERR_INVALID_ARG, "unknown triage token '%s'", bad.c_str());
+  g_triage_next = t;
+  return SLP_OK;
+}
 const char* slp_version(void) { return "slpmoe 0.3 (sm_100a; abi 3)"; }
 
 
@@ -1354,7 +1377,7 @@ slp_status slp_moe_layer_destroy(slp_moe_layer* h) {
   if (!h) return SLP_OK;
   cudaSetDevice(h->cfg.device);
   cudaDeviceSynchronize();
-  const slp_status guard_status = check_guards(h);  // reported by destroy too (SLP_TRIAGE=guards)
+  const slp_status guard_status = check_guards(h);  // reported by destroy too (triage "guards")
   free_pool(h);
   if (h->cur_layer >= 0 && h->cur_layer < static_cast<int>(h->layers.size())) stash_layer(h, h->cur_layer);
   for (LayerW& w : h->layers) {

@@ -234,7 +234,7 @@ def test_cfg2_resident_soak_is_bitwise_stable(dsv3):
 
 
 def test_cfg2_cta_pair_kernel_full_size(dsv3):
-    """The cta_group::2 variant (SLP_TRIAGE gemm=pair) at full size: resident 32K pass against the oracle on
+    """The cta_group::2 variant (triage "gemm=pair") at full size: resident 32K pass against the oracle on
     the tile-boundary tokens, and streamed with empty launch groups impossible here but 64-expert groups."""
     W, Wn = dsv3
     cfg = inputs.CONFIGS[2]

@@ -1,4 +1,4 @@
-"""Memory-safety evidence without compute-sanitizer (closed on the GPU pool): with SLP_TRIAGE=guards every workspace
+"""Memory-safety evidence without compute-sanitizer (closed on the GPU pool): with triage "guards" every workspace
 buffer of a handle sits between two 4 KB canary bands; slp_moe_get_stats and slp_moe_layer_destroy fail if a kernel
 wrote into one.  Reduced layers in every kernel variant and residency, ragged token counts, and the full-size
 DeepSeek-V3-shaped layer (cfg 1 streamed, T = 4096: every tile of every expert is ragged; cfg 2's first 16K tokens

@@ -121,7 +121,7 @@ def test_layer_parity_tcgen05(name, mode):
 
 @pytest.mark.parametrize("name", list(CASES))
 def test_layer_parity_tcgen05_cta_pair(name):
-    """SLP_TRIAGE gemm=pair: the cta_group::2 variant (clusters of two CTAs, pairs of 128-row tiles, dummy
+    """triage "gemm=pair": the cta_group::2 variant (clusters of two CTAs, pairs of 128-row tiles, dummy
     tile for experts with an odd tile count)."""
     check(name, "resident", triage="gemm=pair")
 
@@ -129,7 +129,7 @@ def test_layer_parity_tcgen05_cta_pair(name):
 @pytest.mark.parametrize("name", list(CASES))
 @pytest.mark.parametrize("mode", ["resident", "streamed"])
 def test_layer_parity_tcgen05_static_tiles(name, mode):
-    """SLP_TRIAGE gemm=static: the one-CTA kernel with the static round-robin tile order."""
+    """triage "gemm=static": the one-CTA kernel with the static round-robin tile order."""
     check(name, mode, triage="gemm=static")
 
 

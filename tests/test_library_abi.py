@@ -137,3 +137,12 @@ def test_query_plan_rejects_bad_options(built):
         with pytest.raises(binding.SlpError) as ei:
             binding.query_plan(cfg, **kw)
         assert ei.value.status == -1, kw
+
+
+def test_triage_is_a_thread_local_debug_call_not_an_environment_variable(built):
+    assert built.slp_moe_debug_set_triage(b"gemm=pair,router=fp32,guards") == 0
+    assert built.slp_moe_debug_set_triage(b"gemm=fast") == -1
+    assert b"gemm=fast" in built.slp_last_error()
+    assert built.slp_moe_debug_set_triage(None) == 0          # back to the product path
+    blob = open(binding.library_path(), "rb").read()
+    assert b"SLP_TRIAGE" not in blob      # (getenv itself stays imported: the static CUDA runtime uses it)
