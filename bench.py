@@ -245,7 +245,7 @@ def dry_run_main(args, rank, world):
                           "ms_per_step": ms, "higher_is_better": True, "scaling": "weak" if args.parallelism == "token" else "strong",
                           "vs_baseline": None, "dtype": "none (dry run)", "data": "none (dry run)", "dry_run": True,
                           "config": {"workload": args.workload, "parallelism": f"{args.parallelism} x{world}"}}))
-    if world > 1:
+    if world > 1 or par == "smallep":
         dist.destroy_process_group()
     return 0
 
@@ -284,7 +284,7 @@ def main(argv=None):
     cfg_id, mode = WORKLOADS[args.workload]
     cfg = inputs.CONFIGS[cfg_id]
     ncores = len(os.sched_getaffinity(0))
-    par = args.parallelism if world > 1 else "token"
+    par = args.parallelism   # smallep with one GPU: a one-rank NCCL group, so the collective calls run (as copies) and are timed
     config = {"workload": args.workload, "config": cfg.name, "T": cfg.T, "hidden": cfg.H, "n_experts": cfg.E,
               "top_k": cfg.k, "n_group": cfg.G, "topk_group": cfg.Gk, "moe_intermediate": cfg.I,
               "n_shared": cfg.n_shared, "mode": mode,
@@ -329,6 +329,13 @@ def main(argv=None):
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
+    elif par == "smallep":
+        import socket
+        import torch.distributed as dist
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        dist.init_process_group("nccl", init_method=f"tcp://127.0.0.1:{port}", rank=0, world_size=1, device_id=dev)
     peaks = load_peaks()
     stream = torch.cuda.current_stream()
 
@@ -348,7 +355,7 @@ def main(argv=None):
         hidden = inputs.make_hidden(cfg, device=dev)[t0:t1].contiguous()        # this rank's token shard of the SAME prompt
         layer = SlpMoeLayer(cfg, W, device=local_rank, staging_slots=args.staging_slots, experts_per_launch=args.experts_per_launch,
                             expert_range=(e0, e1), triage=args.triage)
-        runner = smallep.SmallEpLayer(layer, cfg, rank, world)
+        runner = smallep.SmallEpLayer(layer, cfg, rank, world, always_collective=True)
         tokens_this_rank = t1 - t0
     else:
         W = inputs.make_weights(cfg, device=dev, pin=True)
@@ -593,7 +600,7 @@ def main(argv=None):
                           "vs_baseline": None, "dtype": "e4m3 x e4m3 -> f32", "data": "synthetic", "config": config,
                           "clocks": clocks, "e2e": e2e, "gpu_launches": gpu_launches, "roofline": roofline,
                           "cpu_baseline": cpu_baseline, **extra}))
-    if world > 1:
+    if world > 1 or par == "smallep":
         dist.destroy_process_group()
     return 0
 

@@ -30,8 +30,12 @@ class SmallEpLayer:
     """Drives one expert-sharded SlpMoeLayer handle per rank.  `layer` must have been created with
     expert_range=expert_range(E, rank, world)."""
 
-    def __init__(self, layer, cfg, rank, world, group=None):
+    def __init__(self, layer, cfg, rank, world, group=None, always_collective=False):
+        """`always_collective`: issue the all-gather and the reduce-scatter for world == 1 too (a one-rank process
+        group must then exist).  They are copies there, but they are the very calls the multi-rank path makes, so
+        a single GPU can execute and time them."""
         self.layer, self.cfg, self.rank, self.world, self.group = layer, cfg, rank, world, group
+        self.collective = world > 1 or always_collective
         self._all = None
         self._partial = None
         self._mine = None
@@ -44,13 +48,13 @@ class SmallEpLayer:
             self._all = torch.empty((T, H), dtype=torch.bfloat16, device=hidden_shard.device)
             self._partial = torch.empty((T, H), dtype=torch.float32, device=hidden_shard.device)
             self._mine = torch.empty((n, H), dtype=torch.float32, device=hidden_shard.device)
-        if self.world > 1:
+        if self.collective:
             dist.all_gather_into_tensor(self._all, hidden_shard, group=self.group)                       # step 1
         else:
             self._all.copy_(hidden_shard)
         t0 = self.rank * n
         self.layer.prefill_partial(self._all, self._partial, shared_tokens=(t0, t0 + n))                 # steps 2-3
-        if self.world > 1:
+        if self.collective:
             dist.reduce_scatter_tensor(self._mine, self._partial, op=dist.ReduceOp.SUM, group=self.group)  # step 4
         else:
             self._mine.copy_(self._partial)

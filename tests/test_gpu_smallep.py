@@ -118,3 +118,30 @@ def test_bad_expert_ranges_are_rejected():
         with pytest.raises(SlpError) as ei:
             SlpMoeLayer(cfg, W, device=0, expert_range=rng)
         assert ei.value.status == -1
+
+
+def test_one_rank_nccl_group_runs_the_collectives():
+    """The NCCL lines of SmallEpLayer (all_gather_into_tensor on bf16, reduce_scatter_tensor on fp32, then
+    slp_moe_finalize_partial) executed on a real process group of one rank: with one rank they move the data unchanged,
+    so the result must be slp_moe_prefill's bit for bit."""
+    import socket
+    import torch.distributed as dist
+    cfg, W, hidden, ref = problem("mini_dsv3_ragged")
+    x = hidden.cuda()
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    dist.init_process_group("nccl", init_method=f"tcp://127.0.0.1:{port}", rank=0, world_size=1,
+                            device_id=torch.device("cuda", 0))
+    layer = SlpMoeLayer(cfg, W, device=0)
+    try:
+        a = layer.prefill(x).clone()
+        runner = smallep.SmallEpLayer(layer, cfg, 0, 1, always_collective=True)
+        assert runner.collective
+        b = runner.prefill(x).clone()
+        c = runner.prefill(x).clone()      # second call reuses the gathered / partial buffers
+        torch.cuda.synchronize()
+    finally:
+        layer.close()
+        dist.destroy_process_group()
+    assert torch.equal(a.view(torch.int16), b.view(torch.int16)) and torch.equal(b.view(torch.int16), c.view(torch.int16))
