@@ -263,6 +263,91 @@ def measure_fp8_dense_peak(dev, sustained_seconds=3.0):
         return {"error": repr(ex)}
 
 
+def stack_main(args, local_rank):
+    """--workload cfg1_stack / cfg2_stack: a multi-layer stack of DeepSeek-V3-shaped layers on one GPU, streamed through ONE
+    ring of expert slots shared by the layers (PAPER.md:138-144, Fig. 5; slp_moe_stack_*).  A step = one layer call;
+    K steps walk the layers round-robin back to back on one stream, so every call finds the loader already running
+    ahead with its experts.  Reports steady-state ms per layer against the host link, what was prefetched, and the
+    implied whole-model figure (context only)."""
+    import dataclasses
+    import torch
+    import __graft_entry__ as entry
+    entry.build()
+    from paper_2606_10493_b200 import SlpMoeLayer, inputs, measure_h2d_gbs
+    n_layers = args.stack_layers
+    cfg = inputs.CONFIGS[1 if args.workload == "cfg1_stack" else 2]
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    numa = bind_to_gpu_numa_node(local_rank)
+    t0 = time.perf_counter()
+    Ws = [inputs.make_weights(dataclasses.replace(cfg, seed=cfg.seed + 100 * l), device=dev, pin=True) for l in range(n_layers)]
+    hidden = inputs.make_hidden(cfg, device=dev)
+    t_gen = time.perf_counter() - t0
+    h2d_peak = max(measure_h2d_gbs(local_rank, cfg.I * cfg.H, 1 << 30, 5), measure_h2d_gbs(local_rank, 256 << 20, 1 << 30, 5))
+    stack = SlpMoeLayer(cfg, Ws, device=local_rank, staging_slots=args.staging_slots, experts_per_launch=args.experts_per_launch)
+    out = torch.empty_like(hidden)
+    per_layer_bytes = cfg.E * 3 * cfg.I * cfg.H
+    try:
+        for i in range(max(args.warmup, n_layers)):          # at least one full walk, so the steady state is reached
+            stack.prefill(hidden, out, layer=i % n_layers)
+        torch.cuda.synchronize()
+        first = max(args.warmup, n_layers)
+        sampler = ClockSampler(local_rank)
+        sampler.start()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+        stats = []
+        ev[0].record()
+        for i in range(args.steps):
+            stack.prefill(hidden, out, layer=(first + i) % n_layers)
+            ev[i + 1].record()                                # no stats() here: it waits for the call and would serialise the walk
+        # The window opens with one layer already loaded (the warm-up's last call prefetched it) and every call enqueues the
+        # next layer's copies, so it has to close when the LAST call's prefetch has landed too: then exactly K weight
+        # passes crossed the link inside it.  Closing at the last call's compute would count K - 1 passes as K.
+        torch.cuda.synchronize()                              # all streams of the device, the library's copy stream included
+        ev_end = torch.cuda.Event(enable_timing=True)
+        ev_end.record()
+        torch.cuda.synchronize()
+        stats.append(stack.stats())                           # the last call of the back-to-back walk
+        clocks = sampler.stop()
+        per_call = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
+        ms = ev[0].elapsed_time(ev_end) / args.steps
+        iso = []                                              # same walk with a device synchronise between calls
+        for i in range(n_layers):
+            stack.prefill(hidden, out, layer=(first + args.steps + i) % n_layers)
+            torch.cuda.synchronize()
+            iso.append(stack.stats())
+    finally:
+        stack.close()
+    gbs = per_layer_bytes / (ms * 1e-3) / 1e9
+    line = {"metric": METRIC, "value": cfg.T / (ms * 1e-3), "unit": "tokens/s", "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, n_layers),
+            "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "e4m3 x e4m3 -> f32",
+            "data": "synthetic", "clocks": clocks, "e2e": None,
+            "gpu_launches": int(statistics.mean(s["kernel_launches"] for s in stats + iso)),
+            "config": {"workload": args.workload, "config": cfg.name, "T": cfg.T, "layers": n_layers, "mode": "streamed, one ring shared by the layers",
+                       "pinned_host_gb": n_layers * per_layer_bytes / 1e9, "numa": numa, "l2": "inputs_exceed_l2",
+                       "step": "one layer call; layers walked round-robin back to back on one stream"},
+            "link_roofline": {"bound": "host_link", "bytes_per_step": per_layer_bytes, "peak": h2d_peak, "unit": "GB/s",
+                              "achieved_whole_step": gbs, "frac": gbs / h2d_peak},
+            "per_call_ms": {"first": per_call[0], "steady_mean": statistics.mean(per_call[1:]) if len(per_call) > 1 else None,
+                            "steady_min": min(per_call[1:]) if len(per_call) > 1 else None, "steady_max": max(per_call[1:]) if len(per_call) > 1 else None,
+                            "note": "call-to-call CUDA events on the caller's stream; the first timed call finds its layer loaded by the warm-up, "
+                                    "every later one waits for the pass its predecessor started"},
+            "prefetch": {"experts_from_prefetch_per_call": statistics.mean(s["experts_from_prefetch"] for s in stats + iso),
+                         "experts_copied_by_the_call_itself": statistics.mean(s["experts_copied"] for s in stats + iso),
+                         "bytes_prefetched_per_call": statistics.mean(s["bytes_prefetched"] for s in stats + iso),
+                         "note": "counters of the last back-to-back call and of the isolated walk"},
+            "isolated_call": {"ms_total": [s["ms_total"] for s in iso], "ms_route": [s["ms_route"] for s in iso],
+                              "ms_experts": [s["ms_experts"] for s in iso], "ms_combine": [s["ms_combine"] for s in iso],
+                              "note": "device synchronise between calls: the next layer's copies have been running since the previous call was "
+                                      "enqueued, so an isolated call is SHORTER than a weight pass"},
+            "whole_model_context": {"layers": 58, "tokens_per_s": cfg.T / (58 * ms * 1e-3),
+                                    "note": "58 MoE layers at this per-layer time, MoE layers only (no attention); the paper reports "
+                                            "1,200 tok/s for the whole model on its own hardware (context, not a comparison)"},
+            "gen_seconds": t_gen}
+    print(json.dumps(line))
+    return 0
+
+
 def dry_run_main(args, rank, world):
     """CPU-only rank plumbing: gloo rendezvous, the same reductions, rank-0 JSON (no GPU work, fixed numbers)."""
     import torch.distributed as dist
@@ -289,7 +374,7 @@ def main(argv=None):
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="cfg1_streamed", choices=sorted(WORKLOADS))
+    ap.add_argument("--workload", default="cfg1_streamed", choices=sorted(WORKLOADS) + ["cfg1_stack", "cfg2_stack"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--parallelism", default="token", choices=["token", "smallep"])
     ap.add_argument("--dry-run", action="store_true", help="CPU-only rank plumbing check (gloo), no GPU work")
@@ -298,6 +383,7 @@ def main(argv=None):
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
     ap.add_argument("--cpu-baseline-sample", action="store_true", help="cpu_baseline from the bounded, extrapolated sample only (skips the timed full oracle pass)")
     ap.add_argument("--triage", default=None, help="triage spec (slp_moe_debug_set_triage) for A/B runs (e.g. gemm=pair); not a product option")
+    ap.add_argument("--stack-layers", type=int, default=3, help="layers of the cfg1_stack / cfg2_stack workloads")
     ap.add_argument("--staging-slots", type=int, default=0)
     ap.add_argument("--experts-per-launch", type=int, default=0)
     args = ap.parse_args(argv)
@@ -310,6 +396,11 @@ def main(argv=None):
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if args.dry_run:
         return dry_run_main(args, rank, world)
+    if args.workload in ("cfg1_stack", "cfg2_stack"):
+        if world != 1 or args.impl != "ours":
+            print(json.dumps({"error": "the stack workloads run on one GPU, our arm only"}))
+            return 2
+        return stack_main(args, local_rank)
 
     import numpy as np
     import torch
